@@ -1,0 +1,248 @@
+"""Pins P4, P5, P14-P18 of the oracle's likelihood chain (eqs. 2, 3, 11)."""
+import math
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+from oracle import likelihood as L
+from oracle import spline
+from oracle.constants import MODES, YEAR_JULIAN_S
+from oracle.phenom import Intrinsic
+from paper_2005_01827_b200 import workloads as W
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "paper_tables.txt")) as fh:
+    for line in fh:
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            GOLD[line[0]] = float(line[1])
+
+
+@pytest.fixture(scope="module")
+def small(table):
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    return W.build(0, tf, n_bins=8192, batch=3)
+
+
+def test_p4_eq2_identity(table, small):
+    # eq. 2: -1/2 <d-h|d-h> == <d|h> - 1/2 <h|h> - 1/2 <d|d>
+    for b in range(3):
+        dh, hh, logl = L.loglike_parts(table, small["params"][b], small["freqs"], small["data"], small["psd"], small["S"])
+        direct = L.loglike_direct_residual(table, small["params"][b], small["freqs"], small["data"], small["psd"], small["S"])
+        w = L.weights(small["freqs"], small["psd"])
+        dd = L.inner(small["data"], small["data"], w)
+        assert abs(logl - direct) <= 1e-12 * (dd + hh)
+
+
+def test_p5_distance_scaling_and_zero_noise_injection(table):
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    wl = W.build(0, tf, n_bins=8192, batch=2, with_noise=False)
+    p = wl["injections"][0].copy()
+    dh, hh, logl = L.loglike_parts(table, p, wl["freqs"], wl["data"], wl["psd"], wl["S"])
+    assert hh > 1.0 and abs(logl) < 1e-6                    # logL = 0 at the injection, noise-free
+    assert abs(dh - hh) <= 1e-12 * hh
+    for kappa in (0.5, 3.0):
+        p2 = p.copy()
+        p2[4] *= kappa
+        _, hh2, _ = L.loglike_parts(table, p2, wl["freqs"], wl["data"], wl["psd"], wl["S"])
+        assert abs(hh2 * kappa ** 2 / hh - 1.0) < 1e-12      # "D_L is factored into h_lm"
+    # a perturbed walker has logL < 0
+    p3 = p.copy()
+    p3[0] *= 1.0 + 1e-4
+    assert L.loglike_parts(table, p3, wl["freqs"], wl["data"], wl["psd"], wl["S"])[2] < -1.0
+
+
+def test_domain_errors_and_empty_band(table, small):
+    bad = small["params"][0].copy()
+    bad[4] = -1.0
+    assert L.loglike_parts(table, bad, small["freqs"], small["data"], small["psd"], small["S"])[2] == -math.inf
+    # a 1e9 Msun binary has every band below this grid: valid walker, no signal -> logL = -1/2 <d|d>
+    heavy = small["params"][0].copy()
+    heavy[0] = 1e10
+    dh, hh, logl = L.loglike_parts(table, heavy, small["freqs"], small["data"], small["psd"], small["S"])
+    w = L.weights(small["freqs"], small["psd"])
+    assert dh == 0.0 and hh == 0.0 and logl == -0.5 * L.inner(small["data"], small["data"], w)
+    # PSD zeros and non-finite values get weight 0 (G6)
+    psd = small["psd"].copy()
+    psd[0, 5] = 0.0
+    psd[1, 7] = np.inf
+    psd[2, 9] = np.nan
+    w2 = L.weights(small["freqs"], psd)
+    assert w2[0, 5] == 0.0 and w2[1, 7] == 0.0 and w2[2, 9] == 0.0 and np.all(np.isfinite(w2))
+
+
+def test_p14_spline_template_equals_direct_evaluation(table):
+    # north_star pin: spline-interpolated template vs per-bin waveform+response, 1e-8 relative, on a
+    # narrow one-octave grid that keeps every mode on its inspiral branch (no C1 kinks inside)
+    T_s = 2.0e6
+    freqs = (np.arange(2048) + 2000.0) / T_s                 # 1.0e-3 .. 2.02e-3 Hz
+    p = np.array([3e5, 1.7, 0.4, -0.2, 5.0, 1.3, 0.9, 2.2, 0.5, 0.8, 1.5e6])
+    hs = L.template(table, p, freqs, 1024, mode="spline")
+    hd = L.template(table, p, freqs, 1024, mode="direct")
+    for c in range(3):
+        assert np.max(np.abs(hs[c] - hd[c])) <= 1e-8 * np.max(np.abs(hd[c]))
+    assert np.max(np.abs(hd)) > 0.0
+    # and the approximation is visibly worse with few knots (so the test can fail)
+    hc = L.template(table, p, freqs, 16, mode="spline")
+    assert np.max(np.abs(hc[0] - hd[0])) > 1e-6 * np.max(np.abs(hd[0]))
+
+
+def test_p14b_full_band_spline_vs_direct_is_close(table, small):
+    # across the C1 kinks of the model the spline is still a good approximation (not 1e-8)
+    p = small["params"][0]
+    hs = L.template(table, p, small["freqs"], 256, mode="spline")
+    hd = L.template(table, p, small["freqs"], 256, mode="direct")
+    assert np.max(np.abs(hs - hd)) < 2e-2 * np.max(np.abs(hd))
+
+
+def test_p15_exact_linear_phase_term():
+    # theta = Phi - 2 pi f t_coal reduced mod 2 pi must match multi-precision evaluation to 1e-11 rad
+    mp.mp.dps = 60
+    rng = np.random.default_rng(15)
+    df = 1.0 / (1.33 * YEAR_JULIAN_S)
+    k = rng.integers(1, 4_197_160, size=64)
+    f = k.astype(np.float64) * df
+    t_coal = 3.98e7 + rng.uniform(0, 1e5)
+    Phi = rng.uniform(-2e5, 2e5, size=64)
+    out = L._combine(np.ones(64), Phi, [np.ones(64, dtype=np.complex128)], f, t_coal)[0]
+    for i in range(64):
+        th = mp.mpf(float(Phi[i])) - 2 * mp.pi * mp.mpf(float(f[i])) * mp.mpf(t_coal)
+        ref = complex(mp.cos(th), mp.sin(th))
+        # |Phi| up to 2e5 rad carries an fp64 rounding of 3e-11 rad by itself
+        assert abs(out[i] - ref) < 6e-11
+
+
+def test_p17_cosmology_matches_paper_tables():
+    for key, z in (("DL_z4", 4.0), ("DL_z2", 2.0), ("DL_z7", 7.0), ("DL_z100", 100.0)):
+        assert abs(W.lum_dist_gpc(z) / GOLD[key] - 1.0) < 4e-3
+    assert abs(W.lum_dist_gpc(0.01) - GOLD["DL_z0.01"]) < 1e-3
+
+
+def test_p18_tiny_case_against_mpmath(table):
+    """Independent multi-precision re-evaluation of a tiny case: PhenomD inspiral phase and its derivative
+    (formulas retyped in mpmath, derivative by mp.diff), the not-a-knot spline from its defining
+    continuity conditions (dense solve), and the inner-product sums."""
+    mp.mp.dps = 40
+    M, q, a1, a2, D = 1e6, 2.0, 0.3, -0.1, 10.0
+    I = Intrinsic(table, M, q, a1, a2, D)
+    m1, m2 = mp.mpf(2) / 3, mp.mpf(1) / 3
+    eta, delta = m1 * m2, m1 - m2
+    xs, xa = (mp.mpf(a1) + mp.mpf(a2)) / 2, (mp.mpf(a1) - mp.mpf(a2)) / 2
+    pi = mp.pi
+
+    def psi_tf2(f):
+        v = (pi * f) ** (mp.mpf(1) / 3)
+        c2 = mp.mpf(3715) / 756 + 55 * eta / 9
+        c3 = -16 * pi + 113 * delta * xa / 3 + (mp.mpf(113) / 3 - 76 * eta / 3) * xs
+        c4 = (mp.mpf(15293365) / 508032 + 27145 * eta / 504 + 3085 * eta ** 2 / 72
+              + (mp.mpf(-405) / 8 + 200 * eta) * xa ** 2 - mp.mpf(405) / 4 * delta * xa * xs
+              + (mp.mpf(-405) / 8 + 5 * eta / 2) * xs ** 2)
+        c5 = (1 + mp.log(pi * f)) * (38645 * pi / 756 - 65 * pi * eta / 9
+                                      + delta * (mp.mpf(-732985) / 2268 - 140 * eta / 9) * xa
+                                      + (mp.mpf(-732985) / 2268 + 24260 * eta / 81 + 340 * eta ** 2 / 9) * xs)
+        c6 = (mp.mpf(11583231236531) / 4694215680 - 6848 * mp.euler / 21 - 640 * pi ** 2 / 3
+              + (mp.mpf(-15737765635) / 3048192 + 2255 * pi ** 2 / 12) * eta + 76055 * eta ** 2 / 1728
+              - 127825 * eta ** 3 / 1296 - mp.mpf(6848) / 63 * mp.log(64 * pi * f)
+              + 2270 * pi / 3 * delta * xa + (2270 * pi / 3 - 520 * pi * eta) * xs)
+        c7 = (77096675 * pi / 254016 + 378515 * pi * eta / 1512 - 74045 * pi * eta ** 2 / 756
+              + delta * (mp.mpf(-25150083775) / 3048192 + 26804935 * eta / 6048 - 1985 * eta ** 2 / 48) * xa
+              + (mp.mpf(-25150083775) / 3048192 + 10566655595 * eta / 762048 - 1042165 * eta ** 2 / 3024
+                 + 5345 * eta ** 3 / 36) * xs)
+        series = 1 + c2 * v ** 2 + c3 * v ** 3 + c4 * v ** 4 + c5 * v ** 5 + c6 * v ** 6 + c7 * v ** 7
+        ins = (mp.mpf(I.sigma1) * f + mp.mpf(3) / 4 * mp.mpf(I.sigma2) * f ** (mp.mpf(4) / 3)
+               + mp.mpf(3) / 5 * mp.mpf(I.sigma3) * f ** (mp.mpf(5) / 3) + mp.mpf(I.sigma4) / 2 * f ** 2) / eta
+        return -pi / 4 + 3 / (128 * eta) * v ** -5 * series + ins
+
+    for f0 in (2e-4, 3e-3, 0.015):
+        psi, dpsi = I._psi_ins_raw(np.float64(f0))
+        ref = psi_tf2(mp.mpf(f0))
+        dref = mp.diff(psi_tf2, mp.mpf(f0))
+        assert abs(float(psi) - float(ref)) <= 4e-15 * abs(float(ref)) * 8
+        assert abs(float(dpsi) - float(dref)) <= 1e-13 * abs(float(dref))
+
+    # not-a-knot spline from its definition: piecewise cubics, C2 at interior knots, C3 at knots 1 and S-2
+    x = np.array([1.0, 1.3, 1.9, 2.2, 3.1, 3.5, 4.4, 5.0])
+    y = np.array([0.2, -1.0, 0.7, 2.0, 1.1, -0.3, 0.5, 0.9])
+    n = x.size - 1
+    A = mp.zeros(4 * n)
+    b = mp.zeros(4 * n, 1)
+    row = 0
+    for j in range(n):
+        h = mp.mpf(float(x[j + 1])) - mp.mpf(float(x[j]))
+        A[row, 4 * j] = 1; b[row] = mp.mpf(float(y[j])); row += 1
+        for p_ in range(4):
+            A[row, 4 * j + p_] = h ** p_
+        b[row] = mp.mpf(float(y[j + 1])); row += 1
+    for j in range(n - 1):
+        h = mp.mpf(float(x[j + 1])) - mp.mpf(float(x[j]))
+        A[row, 4 * j + 1] = 1; A[row, 4 * j + 2] = 2 * h; A[row, 4 * j + 3] = 3 * h ** 2; A[row, 4 * (j + 1) + 1] = -1; row += 1
+        A[row, 4 * j + 2] = 2; A[row, 4 * j + 3] = 6 * h; A[row, 4 * (j + 1) + 2] = -2; row += 1
+    A[row, 3] = 1; A[row, 7] = -1; row += 1
+    A[row, 4 * (n - 2) + 3] = 1; A[row, 4 * (n - 1) + 3] = -1; row += 1
+    sol = mp.lu_solve(A, b)
+    coef = spline.coefficients(x, y)
+    for j in range(n):
+        for p_ in range(4):
+            assert abs(coef[j, p_] - float(sol[4 * j + p_])) < 1e-12
+
+    # inner products of a tiny case re-summed in multi-precision
+    T_s = 2.0e6
+    freqs = (np.arange(64) + 2000.0) / T_s
+    par = np.array([3e5, 1.7, 0.4, -0.2, 5.0, 1.3, 0.9, 2.2, 0.5, 0.8, 1.5e6])
+    psd = W.scird_psd_aet(freqs)
+    rng = np.random.default_rng(18)
+    data = L.template(table, par, freqs, 16) + W.noise(rng, psd, 1.0 / T_s)
+    h = L.template(table, par * (1 + 1e-5), freqs, 16)
+    dh, hh, logl = L.loglike_parts(table, par * (1 + 1e-5), freqs, data, psd, 16)
+    df = (mp.mpf(float(freqs[-1])) - mp.mpf(float(freqs[0]))) / 63
+    s_dh = s_hh = s_dd = mp.mpf(0)
+    for c in range(3):
+        for k in range(64):
+            w = 4 * df / mp.mpf(float(psd[c, k]))
+            d, hk = data[c, k], h[c, k]
+            s_dh += w * (mp.mpf(d.real) * mp.mpf(hk.real) + mp.mpf(d.imag) * mp.mpf(hk.imag))
+            s_hh += w * (mp.mpf(hk.real) ** 2 + mp.mpf(hk.imag) ** 2)
+            s_dd += w * (mp.mpf(d.real) ** 2 + mp.mpf(d.imag) ** 2)
+    assert abs(dh - float(s_dh)) <= 1e-13 * abs(float(s_dh)) + 1e-13 * float(s_hh)
+    assert abs(hh - float(s_hh)) <= 1e-13 * float(s_hh)
+    assert abs(logl - float(s_dh - s_hh / 2 - s_dd / 2)) <= 1e-12 * float(s_dd + s_hh)
+
+
+def test_band_and_knots(table):
+    # O5: f_lo is the root of t_lm(f) = 0, knots are log-spaced with exact end points
+    p = np.array([1e6, 3.0, 0.6, -0.3, 15.93, 1.0, 1.0, 2.0, 0.3, 0.5, 2.0e6])
+    I = Intrinsic(table, *p[:5])
+    for (l, m) in MODES:
+        band = L.mode_band(I, l, m, p[10], 1e-5, 0.1)
+        assert band is not None
+        t_lo = float(I.t_of_f(l, m, np.float64(band[0]), p[10]))
+        assert abs(t_lo) < 1e-6 * p[10]
+        assert band[1] == pytest.approx(min(0.1, 0.2 * max(1.0, 0.5 * m) / I.M_s))
+        k = L.knots_for_band(band[0], band[1], 256)
+        assert k[0] == band[0] and k[-1] == band[1] and np.all(np.diff(k) > 0)
+        r = k[1:] / k[:-1]
+        assert np.max(np.abs(r / r[0] - 1.0)) < 1e-12
+    # modes of lower m start later in frequency: f_lo scales like m at fixed t
+    b22 = L.mode_band(I, 2, 2, p[10], 1e-5, 0.1)[0]
+    b44 = L.mode_band(I, 4, 4, p[10], 1e-5, 0.1)[0]
+    b21 = L.mode_band(I, 2, 1, p[10], 1e-5, 0.1)[0]
+    assert b44 == pytest.approx(2.0 * b22, rel=1e-9) and b21 == pytest.approx(0.5 * b22, rel=1e-9)
+
+
+def test_p16_soft_snr_of_paper_binaries(table):
+    # Soft pin only (model numbers are surrogates, no Galactic confusion noise): the optimal SNR of
+    # Table II Binary 1 with t0 = 1 yr must come out at the right order of magnitude.
+    freqs = 1e-4 + 2e-7 * np.arange(1 << 17)              # coarse uniform grid up to 26 mHz (|h|^2/S_n is smooth)
+    psd = W.scird_psd_aet(freqs)
+    p = np.array([2e6, 1.0 / 3.0, 0.0, 0.0, 36.59, 2.14, 1.05, -0.024, 0.62, 2.03, 50.25])
+    h = L.template(table, p, freqs, 1024, t0=YEAR_JULIAN_S)
+    snr = math.sqrt(L.inner(h, h, L.weights(freqs, psd)))
+    print("Binary 1 optimal SNR (surrogate model, SciRD w/o confusion, f > 1e-4 Hz):", snr, "paper:", GOLD["SNR_binary1"])
+    assert GOLD["SNR_binary1"] / 3.0 < snr < GOLD["SNR_binary1"] * 3.0
+    # mode mixing: the total is not the quadrature sum of the isolated modes
+    parts = [math.sqrt(L.inner(hm, hm, L.weights(freqs, psd)))
+             for hm in (L.template(table, p, freqs, 1024, t0=YEAR_JULIAN_S, mode_mask=1 << i) for i in range(6))]
+    print("per-mode SNR:", parts)
+    assert parts[0] == max(parts) and abs(math.sqrt(sum(x * x for x in parts)) - snr) > 1e-3 * snr
