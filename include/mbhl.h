@@ -1,0 +1,136 @@
+/* mbhl.h - C ABI of the B200-native batched LISA massive-black-hole-binary log-likelihood.
+ *
+ * Implements the likelihood hot path of arXiv:2005.01827 (section II.A):
+ *   one-time upload of the data stream and noise PSD
+ *   per call, for each parameter set ("walker"):
+ *     PhenomHM amplitude/phase of 6 modes on a sparse grid      (eq. 5)
+ *     t_lm(f), frequency bounds                                 (eq. 6)
+ *     fast frequency-domain LISA response, TDI A/E/T            (eqs. 7-10)
+ *     cubic-spline coefficients of the sparse smooth functions
+ *     interpolation to the dense Fourier grid, mode sum, PSD-weighted inner products,
+ *     logL = -1/2 <d-h|d-h> = <d|h> - 1/2 <h|h> - 1/2 <d|d>     (eqs. 2, 3, 11)
+ * All arithmetic is fp64 and runs in hand-written sm_100a CUDA kernels; there is no CPU path.
+ * The readings of the paper that fix what is silent or ambiguous are listed in DESIGN.md section 4.
+ *
+ * Conventions common to all calls
+ *   - Return value: 0 (MBHL_OK) or a negative MBHL_E* code; never throws, never aborts.
+ *     mbhl_last_error(ctx) gives a message for the last failing call on that context.
+ *   - "device pointer" = memory on the context's CUDA device (e.g. torch.Tensor.data_ptr()).
+ *   - Hot-path calls (mbhl_loglike*, mbhl_template, mbhl_sparse) are ASYNCHRONOUS on the
+ *     context's stream; outputs are valid after the caller synchronises that stream.
+ *   - A context is not thread-safe; several contexts may coexist.
+ *   - Parameter vector, 11 doubles per walker, row-major [B][11]:
+ *       0 M_T   total mass, detector frame [solar masses]
+ *       1 q     mass ratio; any q > 0 is accepted, q and 1/q are the same binary (reading G15)
+ *       2 a1    dimensionless aligned spin of the HEAVIER body, |a1| <= 1
+ *       3 a2    dimensionless aligned spin of the lighter body, |a2| <= 1
+ *       4 D_L   luminosity distance [Gpc]
+ *       5 phi_ref  reference phase [rad]
+ *       6 iota  inclination [rad]
+ *       7 lambda   ecliptic longitude, SSB frame [rad]
+ *       8 beta  ecliptic latitude, SSB frame [rad]
+ *       9 psi   polarisation angle [rad]
+ *      10 t_ref reference time [s]; t_coal = t0 + t_ref, t = 0 is the start of the data
+ *   - Per-walker domain errors are not call errors: a walker with a non-finite parameter,
+ *     M_T <= 0, D_L <= 0, q <= 0, |a1| > 1 or |a2| > 1 gets logL = -inf and <d|h> = <h|h> = 0;
+ *     a valid walker whose modes all fall outside the grid gets logL = -1/2 <d|d>.  Never NaN.
+ *   - Mode order everywhere: (2,2),(3,3),(4,4),(2,1),(3,2),(4,3).
+ *   - Splined quantities per (walker, mode), Q = 8, in this order (reading G8):
+ *       0 A_lm [strain*s]; 1 Phi_lm = phi_lm + phi_Doppler without the linear term -2 pi f t_coal;
+ *       2,3 Re,Im That^A; 4,5 Re,Im That^E; 6,7 Re,Im That^T.
+ */
+#ifndef MBHL_H
+#define MBHL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MBHL_OK        0
+#define MBHL_EINVAL   -1   /* null pointer, bad size, non-uniform / non-increasing / non-positive grid   */
+#define MBHL_ENOMEM   -2   /* device or host allocation failed                                           */
+#define MBHL_ECUDA    -3   /* CUDA runtime error, text in mbhl_last_error                                */
+#define MBHL_ENOWS    -4   /* caller-supplied workspace too small for this batch                         */
+
+#define MBHL_NPARAM   11
+#define MBHL_NMODE     6
+#define MBHL_NQ        8
+
+typedef struct mbhl_ctx mbhl_ctx;     /* opaque; owned by the library, released by mbhl_free */
+
+typedef struct mbhl_config {
+    int32_t  sparse_points;  /* S, knots per mode, >= 8; 0 = default 1024 ("~2^10")          */
+    uint32_t mode_mask;      /* bit i enables mode i of the order above; 0 = all six                     */
+    double   t0;             /* t_coal = t0 + t_ref                                       */
+    int64_t  max_batch;      /* hint for the internal workspace; 0 = grow on demand                      */
+    int32_t  device;         /* CUDA device ordinal                                                      */
+    void*    stream;         /* cudaStream_t all work is enqueued on; NULL = legacy default stream       */
+} mbhl_config;
+
+/* One-time setup.  freqs[N]: strictly increasing, uniform (relative tolerance 1e-6 on the
+ * spacing), freqs[0] > 0, N >= 4.  data_AET[3][N][2]: (Re, Im) of d^A, d^E, d^T.  psd_AET[3][N]: one-sided
+ * noise PSD; bins with S_n <= 0 or non-finite get weight 0 (reading G6).  The three arrays may be host or
+ * device pointers (detected); they are copied/transformed into library-owned device buffers
+ * (w = 4 df / S_n with df = (f[N-1]-f[0])/(N-1), w*d, and <d|d>), so the caller may free them afterwards.
+ * cfg == NULL means all defaults on device 0.  On success *out holds the new context.                   */
+int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data_AET,
+              const double* psd_AET, const mbhl_config* cfg);
+
+/* logL[b] for params[b][11], b < B (eq. 2).  params, logL: device pointers, caller-owned.  B >= 0.       */
+int mbhl_loglike(mbhl_ctx* ctx, const double* params, int64_t B, double* logL);
+
+/* Same, also returning <d|h> and <h|h> (either may be NULL); logL = d_h - h_h/2 - <d|d>/2.               */
+int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B,
+                       double* d_h, double* h_h, double* logL);
+
+/* Host-buffer convenience for end-to-end use: params_host[B][11] and logL_host[B] are HOST pointers
+ * (pinned memory makes the copies asynchronous); the call enqueues H2D, the hot path and D2H on the
+ * context's stream and synchronises it before returning.                                               */
+int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, double* logL_host);
+
+/* Template h^{A,E,T} of each walker on freqs_out[Nout] (device pointer; NULL = the init grid, Nout ignored),
+ * written to out_AET[B][3][Nout][2] (device).  direct = 0: the spline path the likelihood uses;
+ * direct = 1: waveform + response evaluated at every bin (no spline).  A mode contributes only inside its
+ * band [f_lo, f_hi] (no extrapolation).  Testing / injection aid (PAPER.md:171 stores this; the
+ * likelihood path never does).                                                                          */
+int mbhl_template(mbhl_ctx* ctx, const double* params, int64_t B, const double* freqs_out,
+                  int64_t Nout, double* out_AET, int32_t direct);
+
+/* Sparse stage only (steps a1-a5).  Any output may be NULL.  Device pointers.
+ *   knots[B][6][S]      log-spaced knots f_s [Hz]; all 0 for an inactive mode
+ *   y[B][6][8][S]       the Q = 8 smooth functions at the knots (Phi in radians)
+ *   coef[B][6][S-1][8][4]  per interval (y_j, s_j, c_j, d_j): p = y_j + s_j u + c_j u^2 + d_j u^3, u = f - f_j.
+ *                       The Phi row is stored in CYCLES (Phi / 2 pi) with y_j reduced into [-1/2, 1/2].    */
+int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, double* y, double* coef);
+
+/* Workspace the hot path needs for a batch of B (bytes).                                                 */
+size_t mbhl_workspace_bytes(const mbhl_ctx* ctx, int64_t B);
+/* Optional caller-owned workspace (device pointer, 256-byte aligned); once set the library performs no
+ * device allocation in the hot path and returns MBHL_ENOWS if it is too small.  NULL returns to internal.*/
+int mbhl_set_workspace(mbhl_ctx* ctx, void* dev_ptr, size_t bytes);
+
+/* Introspection. */
+double  mbhl_data_norm(const mbhl_ctx* ctx);        /* <d|d> computed at init                            */
+int64_t mbhl_num_bins(const mbhl_ctx* ctx);
+int32_t mbhl_sparse_points(const mbhl_ctx* ctx);
+int64_t mbhl_launch_count(const mbhl_ctx* ctx);     /* kernels this context has launched so far          */
+/* Work counters of the last mbhl_loglike* call (device -> host copy, synchronises the stream):
+ * pairs = sum over walkers and modes of in-band bins, bins = sum over walkers of bins covered by >= 1 mode. */
+int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins);
+
+/* FP64 DFMA-chain probe used to measure the roofline denominator: each of blocks*threads threads runs
+ * iters*8 dependent-chain DFMAs (8 independent chains); sink is a device pointer to >= 1 double.
+ * Asynchronous on `stream`.  FLOPs = 2 * blocks * threads * iters * 8.                                   */
+int mbhl_dfma_probe(void* stream, int32_t blocks, int32_t threads, int64_t iters, double* sink);
+
+const char* mbhl_strerror(int code);
+const char* mbhl_last_error(const mbhl_ctx* ctx);
+void mbhl_free(mbhl_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MBHL_H */

@@ -1,0 +1,413 @@
+// mbhl_api.cu - host side of the C ABI declared in include/mbhl.h.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "mbhl.h"
+#include "mbhl_kernels.cuh"
+
+using namespace mbhl;
+
+struct mbhl_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int S = 1024;
+    uint32_t mode_mask = 0x3F;
+    double t0 = 0.0;
+    int64_t N = 0;
+    double f_min = 0.0, f_max = 0.0, df = 0.0, dd = 0.0;
+    // library-owned device data
+    double* freqs = nullptr;
+    double* w = nullptr;
+    double* wdre = nullptr;
+    double* wdim = nullptr;
+    unsigned long long* counters = nullptr;
+    // workspace
+    void* ws_internal = nullptr;
+    size_t ws_internal_bytes = 0;
+    void* ws_user = nullptr;
+    size_t ws_user_bytes = 0;
+    int64_t launches = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+struct WsLayout {
+    size_t params, consts, knots, y, coef, partials, dh, hh, logl, total;
+};
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int n_chunks_of(int64_t N) { return (int)((N + kChunk - 1) / kChunk); }
+
+WsLayout layout(const mbhl_ctx* c, int64_t B) {
+    WsLayout L;
+    size_t off = 0;
+    const size_t b = (size_t)(B > 0 ? B : 1);
+    L.params = off; off += align256(b * MBHL_NPARAM * sizeof(double));
+    L.consts = off; off += align256(b * sizeof(WalkerConst));
+    L.knots = off; off += align256(b * MBHL_NMODE * c->S * sizeof(double));
+    L.y = off; off += align256(b * MBHL_NMODE * MBHL_NQ * c->S * sizeof(double));
+    L.coef = off; off += align256(b * MBHL_NMODE * (size_t)(c->S - 1) * kCoefStride * sizeof(double));
+    L.partials = off; off += align256(b * (size_t)n_chunks_of(c->N) * 2 * sizeof(double));
+    L.dh = off; off += align256(b * sizeof(double));
+    L.hh = off; off += align256(b * sizeof(double));
+    L.logl = off; off += align256(b * sizeof(double));
+    L.total = off;
+    return L;
+}
+
+int fail(mbhl_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
+    if (c) {
+        if (e != cudaSuccess) snprintf(c->err, sizeof(c->err), "%s: %s", what, cudaGetErrorString(e));
+        else snprintf(c->err, sizeof(c->err), "%s", what);
+    }
+    return code;
+}
+
+#define CU(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return fail(ctx, MBHL_ECUDA, #call, e_); \
+    } while (0)
+
+int get_workspace(mbhl_ctx* ctx, int64_t B, char** base) {
+    const size_t need = layout(ctx, B).total;
+    if (ctx->ws_user) {
+        if (ctx->ws_user_bytes < need) return fail(ctx, MBHL_ENOWS, "caller workspace too small for this batch");
+        *base = (char*)ctx->ws_user;
+        return MBHL_OK;
+    }
+    if (ctx->ws_internal_bytes < need) {
+        if (ctx->ws_internal) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->ws_internal);
+            ctx->ws_internal = nullptr;
+            ctx->ws_internal_bytes = 0;
+        }
+        cudaError_t e = cudaMalloc(&ctx->ws_internal, need);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(ctx, MBHL_ENOMEM, "cudaMalloc(workspace)", e);
+        }
+        ctx->ws_internal_bytes = need;
+    }
+    *base = (char*)ctx->ws_internal;
+    return MBHL_OK;
+}
+
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// Runs the sparse stage (a1-a5) for params already on the device.
+int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, const WsLayout& L, bool with_coef) {
+    WalkerConst* wc = (WalkerConst*)(base + L.consts);
+    double* knots = (double*)(base + L.knots);
+    double* y = (double*)(base + L.y);
+    double* coef = (double*)(base + L.coef);
+    const int S = ctx->S;
+    k_walker_consts<<<(unsigned)((B + 63) / 64), 64, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
+                                                                      ctx->mode_mask, wc);
+    dim3 gs((unsigned)(B * MBHL_NMODE), (unsigned)((S + 127) / 128));
+    k_sparse_eval<<<gs, 128, 0, ctx->stream>>>(wc, S, knots, y);
+    ctx->launches += 2;
+    if (with_coef) {
+        k_spline<<<(unsigned)(B * MBHL_NMODE), 128, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
+        ctx->launches += 1;
+    }
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mbhl_strerror(int code) {
+    switch (code) {
+        case MBHL_OK: return "ok";
+        case MBHL_EINVAL: return "invalid argument";
+        case MBHL_ENOMEM: return "out of memory";
+        case MBHL_ECUDA: return "CUDA error";
+        case MBHL_ENOWS: return "workspace too small";
+        default: return "unknown error";
+    }
+}
+
+const char* mbhl_last_error(const mbhl_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+void mbhl_free(mbhl_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->freqs);
+    cudaFree(ctx->w);
+    cudaFree(ctx->wdre);
+    cudaFree(ctx->wdim);
+    cudaFree(ctx->counters);
+    cudaFree(ctx->ws_internal);
+    delete ctx;
+}
+
+int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data_AET, const double* psd_AET,
+              const mbhl_config* cfg) {
+    if (!out) return MBHL_EINVAL;
+    *out = nullptr;
+    if (!freqs || !data_AET || !psd_AET || N < 4) return MBHL_EINVAL;
+    mbhl_ctx* ctx = new (std::nothrow) mbhl_ctx();
+    if (!ctx) return MBHL_ENOMEM;
+    if (cfg) {
+        ctx->device = cfg->device;
+        ctx->stream = (cudaStream_t)cfg->stream;
+        if (cfg->sparse_points) ctx->S = cfg->sparse_points;
+        if (cfg->mode_mask) ctx->mode_mask = cfg->mode_mask & 0x3F;
+        ctx->t0 = cfg->t0;
+    }
+    ctx->N = N;
+    int rc = MBHL_OK;
+    double *d_data = nullptr, *d_psd = nullptr, *d_part = nullptr;
+    std::vector<double> host_part;
+    auto cleanup = [&](int code) {
+        cudaFree(d_data);
+        cudaFree(d_psd);
+        cudaFree(d_part);
+        if (code != MBHL_OK) {
+            cudaFree(ctx->freqs); cudaFree(ctx->w); cudaFree(ctx->wdre); cudaFree(ctx->wdim); cudaFree(ctx->counters);
+            delete ctx;
+        }
+        return code;
+    };
+    if (ctx->S < 8 || ctx->S > 8192 || !isfinite(ctx->t0)) return cleanup(MBHL_EINVAL);
+    if (spline_smem_bytes(ctx->S) > 227 * 1024) return cleanup(MBHL_EINVAL);   // S <= ~1550 fits one CTA's shared memory
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return cleanup(MBHL_ECUDA);
+    if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
+    if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
+    const size_t nb = (size_t)N * sizeof(double);
+    const int nblk = (int)((N + 1023) / 1024);
+    if (cudaMalloc(&ctx->freqs, nb) != cudaSuccess || cudaMalloc(&ctx->w, 3 * nb) != cudaSuccess ||
+        cudaMalloc(&ctx->wdre, 3 * nb) != cudaSuccess || cudaMalloc(&ctx->wdim, 3 * nb) != cudaSuccess ||
+        cudaMalloc(&ctx->counters, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMalloc(&d_part, (size_t)nblk * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return cleanup(MBHL_ENOMEM);
+    }
+    cudaStream_t st = ctx->stream;
+    // freqs
+    if (cudaMemcpyAsync(ctx->freqs, freqs, nb, cudaMemcpyDefault, st) != cudaSuccess) return cleanup(MBHL_ECUDA);
+    const double* data_dev = data_AET;
+    const double* psd_dev = psd_AET;
+    if (!is_device_ptr(data_AET)) {
+        if (cudaMalloc(&d_data, 6 * nb) != cudaSuccess) { cudaGetLastError(); return cleanup(MBHL_ENOMEM); }
+        if (cudaMemcpyAsync(d_data, data_AET, 6 * nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return cleanup(MBHL_ECUDA);
+        data_dev = d_data;
+    }
+    if (!is_device_ptr(psd_AET)) {
+        if (cudaMalloc(&d_psd, 3 * nb) != cudaSuccess) { cudaGetLastError(); return cleanup(MBHL_ENOMEM); }
+        if (cudaMemcpyAsync(d_psd, psd_AET, 3 * nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return cleanup(MBHL_ECUDA);
+        psd_dev = d_psd;
+    }
+    // grid: end points, spacing, validation
+    double ends[2];
+    if (cudaMemcpyAsync(&ends[0], ctx->freqs, sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(&ends[1], ctx->freqs + (N - 1), sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
+    ctx->f_min = ends[0];
+    ctx->f_max = ends[1];
+    ctx->df = (ends[1] - ends[0]) / (double)(N - 1);
+    if (!(ctx->f_min > 0.0) || !(ctx->df > 0.0) || !isfinite(ctx->f_max)) return cleanup(MBHL_EINVAL);
+    host_part.resize(nblk);
+    k_check_grid<<<nblk, 256, 0, st>>>(ctx->freqs, N, ctx->df, d_part);
+    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nblk * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
+    for (int i = 0; i < nblk; ++i)
+        if (!(host_part[i] <= 1e-6)) return cleanup(MBHL_EINVAL);
+    // weights, weighted data, <d|d>
+    k_init_weights<<<nblk, 256, 0, st>>>(data_dev, psd_dev, N, ctx->df, ctx->w, ctx->wdre, ctx->wdim, d_part);
+    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nblk * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
+    ctx->launches += 2;
+    {
+        // pairwise (fixed-order) host sum of the per-block partials
+        std::vector<double> v(host_part);
+        size_t n = v.size();
+        while (n > 1) {
+            size_t h = (n + 1) / 2;
+            for (size_t i = 0; i + h < n; ++i) v[i] += v[i + h];
+            n = h;
+        }
+        ctx->dd = v[0];
+    }
+    if (cfg && cfg->max_batch > 0) {
+        char* base;
+        rc = get_workspace(ctx, cfg->max_batch, &base);
+        if (rc != MBHL_OK) return cleanup(rc);
+    }
+    cleanup(MBHL_OK);
+    *out = ctx;
+    return MBHL_OK;
+}
+
+size_t mbhl_workspace_bytes(const mbhl_ctx* ctx, int64_t B) { return ctx ? layout(ctx, B).total : 0; }
+
+int mbhl_set_workspace(mbhl_ctx* ctx, void* dev_ptr, size_t bytes) {
+    if (!ctx) return MBHL_EINVAL;
+    if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return fail(ctx, MBHL_EINVAL, "workspace must be 256-byte aligned");
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->ws_user = dev_ptr;
+    ctx->ws_user_bytes = dev_ptr ? bytes : 0;
+    return MBHL_OK;
+}
+
+double mbhl_data_norm(const mbhl_ctx* ctx) { return ctx ? ctx->dd : NAN; }
+int64_t mbhl_num_bins(const mbhl_ctx* ctx) { return ctx ? ctx->N : 0; }
+int32_t mbhl_sparse_points(const mbhl_ctx* ctx) { return ctx ? ctx->S : 0; }
+int64_t mbhl_launch_count(const mbhl_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h, double* logL) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
+    if (B == 0) return MBHL_OK;
+    if (B > 65535) {
+        // grid.y limit of the dense kernel: process in slices
+        for (int64_t o = 0; o < B; o += 32768) {
+            const int64_t n = (B - o < 32768) ? (B - o) : 32768;
+            int rc = mbhl_loglike_parts(ctx, params + o * MBHL_NPARAM, n, d_h ? d_h + o : nullptr, h_h ? h_h + o : nullptr,
+                                        logL ? logL + o : nullptr);
+            if (rc != MBHL_OK) return rc;
+        }
+        return MBHL_OK;
+    }
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    rc = run_sparse(ctx, params, B, base, L, true);
+    if (rc != MBHL_OK) return rc;
+    DenseArgs A;
+    A.wc = (const WalkerConst*)(base + L.consts);
+    A.knots = (const double*)(base + L.knots);
+    A.coef = (const double*)(base + L.coef);
+    A.freqs = ctx->freqs;
+    A.w = ctx->w;
+    A.wdre = ctx->wdre;
+    A.wdim = ctx->wdim;
+    A.partials = (double*)(base + L.partials);
+    A.counters = ctx->counters;
+    A.N = ctx->N;
+    A.S = ctx->S;
+    A.n_chunks = n_chunks_of(ctx->N);
+    CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    dim3 gd((unsigned)A.n_chunks, (unsigned)B);
+    k_dense<<<gd, kDenseThreads, 0, ctx->stream>>>(A);
+    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.wc, A.partials, A.n_chunks, B, ctx->dd, d_h, h_h, logL);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+int mbhl_loglike(mbhl_ctx* ctx, const double* params, int64_t B, double* logL) {
+    if (ctx && B > 0 && !logL) return fail(ctx, MBHL_EINVAL, "logL is null");
+    return mbhl_loglike_parts(ctx, params, B, nullptr, nullptr, logL);
+}
+
+int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, double* logL_host) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && (!params_host || !logL_host))) return fail(ctx, MBHL_EINVAL, "bad host buffers");
+    if (B == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    double* p_dev = (double*)(base + L.params);
+    double* l_dev = (double*)(base + L.logl);
+    CU(cudaMemcpyAsync(p_dev, params_host, (size_t)B * MBHL_NPARAM * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    rc = mbhl_loglike_parts(ctx, p_dev, B, nullptr, nullptr, l_dev);
+    if (rc != MBHL_OK) return rc;
+    CU(cudaMemcpyAsync(logL_host, l_dev, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MBHL_OK;
+}
+
+int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins) {
+    if (!ctx) return MBHL_EINVAL;
+    unsigned long long h[2];
+    CU(cudaMemcpyAsync(h, ctx->counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (pairs) *pairs = (int64_t)h[0];
+    if (bins) *bins = (int64_t)h[1];
+    return MBHL_OK;
+}
+
+int mbhl_template(mbhl_ctx* ctx, const double* params, int64_t B, const double* freqs_out, int64_t Nout, double* out_AET,
+                  int32_t direct) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && (!params || !out_AET))) return fail(ctx, MBHL_EINVAL, "bad template arguments");
+    if (!freqs_out) { freqs_out = ctx->freqs; Nout = ctx->N; }
+    if (Nout < 0 || B > 65535) return fail(ctx, MBHL_EINVAL, "bad Nout or B > 65535");
+    if (B == 0 || Nout == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    rc = run_sparse(ctx, params, B, base, L, direct == 0);
+    if (rc != MBHL_OK) return rc;
+    dim3 g((unsigned)((Nout + 127) / 128), (unsigned)B);
+    k_template<<<g, 128, 0, ctx->stream>>>((const WalkerConst*)(base + L.consts), (const double*)(base + L.knots),
+                                           (const double*)(base + L.coef), ctx->S, freqs_out, Nout, out_AET, direct ? 1 : 0);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, double* y, double* coef) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
+    if (B == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    rc = run_sparse(ctx, params, B, base, L, true);
+    if (rc != MBHL_OK) return rc;
+    const size_t nk = (size_t)B * MBHL_NMODE * ctx->S;
+    if (knots) CU(cudaMemcpyAsync(knots, base + L.knots, nk * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    if (y) {
+        const int64_t rows = B * MBHL_NMODE * MBHL_NQ;
+        k_export_y<<<(unsigned)((rows * ctx->S + 255) / 256), 256, 0, ctx->stream>>>((const double*)(base + L.y), rows, ctx->S, y);
+        ctx->launches += 1;
+    }
+    if (coef)
+        CU(cudaMemcpyAsync(coef, base + L.coef, (size_t)B * MBHL_NMODE * (ctx->S - 1) * kCoefStride * sizeof(double),
+                           cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+int mbhl_dfma_probe(void* stream, int32_t blocks, int32_t threads, int64_t iters, double* sink) {
+    if (blocks <= 0 || threads <= 0 || threads > 1024 || iters < 0 || !sink) return MBHL_EINVAL;
+    k_dfma_probe<<<blocks, threads, 0, (cudaStream_t)stream>>>(iters, sink);
+    return cudaGetLastError() == cudaSuccess ? MBHL_OK : MBHL_ECUDA;
+}
+
+}  // extern "C"

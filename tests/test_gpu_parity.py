@@ -1,0 +1,266 @@
+"""GPU parity tests: the CUDA path through the C ABI against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star): |dlogL| <= 1e-6 (1 + |logL|); per-bin template error <= 1e-9
+relative to max|h^c| per channel (G6), band-edge bins excluded (G10).
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import likelihood as L
+from oracle import spline as ospline
+from oracle.constants import MODES
+from oracle.phenom import Intrinsic
+from paper_2005_01827_b200 import binding as M
+from paper_2005_01827_b200 import workloads as W
+
+DEV = "cuda:0"
+
+
+def dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x), device=DEV)
+
+
+def make_ctx(wl, **kw):
+    return M.mbhl_init(dev(wl["freqs"]), dev(wl["data"]), dev(wl["psd"]), sparse_points=wl["S"], t0=wl["t0"], **kw)
+
+
+@pytest.fixture(scope="module")
+def cfg0(table):
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    wl = W.build(0, tf)
+    # extra walkers: equal masses (odd modes vanish), q < 1 (reading G15), extreme spins, a heavy binary
+    extra = wl["params"][:4].copy()
+    extra[0, 1] = 1.0
+    extra[1, 1] = 1.0 / extra[1, 1]
+    extra[2, 2:4] = [-0.99, 0.99]
+    extra[3, 0] = 3e7
+    wl["params"] = np.concatenate([wl["params"], extra])
+    return wl
+
+
+def edge_mask(table, params, freqs, t0):
+    """True for bins within +-1 of any mode's band edge (membership may legitimately differ, G10)."""
+    p = L.unpack(params)
+    intr = Intrinsic(table, p["M_T"], p["q"], p["a1"], p["a2"], p["D_L"])
+    mask = np.zeros(freqs.size, dtype=bool)
+    for (l, m) in MODES:
+        band = L.mode_band(intr, l, m, t0 + p["t_ref"], freqs[0], freqs[-1])
+        if band is None:
+            continue
+        for edge in band:
+            k = int(np.searchsorted(freqs, edge))
+            mask[max(0, k - 2):k + 2] = True
+    return mask
+
+
+def test_sparse_stage_parity(table, cfg0):
+    ctx = make_ctx(cfg0)
+    params = cfg0["params"]
+    knots, y, coef = [t.cpu().numpy() for t in M.mbhl_sparse(ctx, dev(params))]
+    S = cfg0["S"]
+    for b in range(params.shape[0]):
+        modes, _ = L.sparse_stage(table, params[b], cfg0["freqs"][0], cfg0["freqs"][-1], S, cfg0["t0"])
+        for mi, mo in enumerate(modes):
+            if mo is None:
+                assert np.all(knots[b, mi] == 0.0) and np.all(coef[b, mi] == 0.0)
+                continue
+            assert np.max(np.abs(knots[b, mi] / mo["knots"] - 1.0)) < 1e-13
+            yo = mo["y"]
+            amp_scale = np.max(np.abs(yo[0]))
+            if amp_scale > 0:
+                assert np.max(np.abs(y[b, mi, 0] - yo[0])) <= 1e-10 * amp_scale
+            assert np.max(np.abs(y[b, mi, 1] - yo[1])) <= 2e-8                       # radians
+            tscale = np.max(np.abs(yo[2:]))
+            assert np.max(np.abs(y[b, mi, 2:] - yo[2:])) <= 1e-10 * tscale
+            # spline coefficients (phase row in cycles, y_j reduced mod 1)
+            co = mo["coef"].copy()                    # [S-1, 8, 4]
+            co[:, 1, :] /= 2.0 * math.pi
+            cg = coef[b, mi]
+            for q in range(8):
+                for col in range(4):
+                    ref = co[:, q, col]
+                    got = cg[:, q, col]
+                    if q == 1 and col == 0:
+                        d = got - ref
+                        assert np.max(np.abs(d - np.rint(d))) <= 1e-8 and np.max(np.abs(got)) <= 0.5 + 1e-12
+                    else:
+                        scale = np.max(np.abs(ref))
+                        if scale > 0:
+                            assert np.max(np.abs(got - ref)) <= 2e-8 * scale, (b, mi, q, col)
+    M.mbhl_free(ctx)
+
+
+@pytest.mark.parametrize("direct", [False, True])
+def test_template_parity_config0(table, cfg0, direct):
+    ctx = make_ctx(cfg0)
+    params = cfg0["params"]
+    h_gpu = M.mbhl_template(ctx, dev(params), direct=direct).cpu().numpy()
+    for b in range(params.shape[0]):
+        h_ref = L.template(table, params[b], cfg0["freqs"], cfg0["S"], cfg0["t0"], mode="direct" if direct else "spline")
+        keep = ~edge_mask(table, params[b], cfg0["freqs"], cfg0["t0"])
+        for c in range(3):
+            scale = np.max(np.abs(h_ref[c]))
+            assert scale > 0
+            err = np.max(np.abs(h_gpu[b, c][keep] - h_ref[c][keep])) / scale
+            assert err <= 1e-9, (b, c, err)
+        # edge bins: either side's value is a valid one (in or out of band): |diff| bounded by the local amplitude
+        assert np.all(np.abs(h_gpu[b] - h_ref)[:, ~keep] <= 1.0001 * np.maximum(np.abs(h_gpu[b]), np.abs(h_ref))[:, ~keep] + 1e-300)
+    M.mbhl_free(ctx)
+
+
+def test_template_on_another_grid(table, cfg0):
+    ctx = make_ctx(cfg0)
+    f_out = np.sort(np.random.default_rng(5).uniform(cfg0["freqs"][0], cfg0["freqs"][-1], 3001))
+    p = cfg0["params"][:2]
+    h_gpu = M.mbhl_template(ctx, dev(p), freqs_out=dev(f_out)).cpu().numpy()
+    for b in range(2):
+        # the bands come from the init grid; evaluate the oracle's splines at f_out
+        modes, t_coal = L.sparse_stage(table, p[b], cfg0["freqs"][0], cfg0["freqs"][-1], cfg0["S"], cfg0["t0"])
+        h_ref = np.zeros((3, f_out.size), dtype=np.complex128)
+        for mo in modes:
+            if mo is None:
+                continue
+            sel = np.nonzero((f_out >= mo["knots"][0]) & (f_out <= mo["knots"][-1]))[0]
+            q = np.stack([ospline.evaluate(mo["knots"], mo["coef"][:, qi, :], f_out[sel]) for qi in range(8)])
+            That = [q[2] + 1j * q[3], q[4] + 1j * q[5], q[6] + 1j * q[7]]
+            for c, hc in enumerate(L._combine(q[0], q[1], That, f_out[sel], t_coal)):
+                h_ref[c, sel] += hc
+        for c in range(3):
+            assert np.max(np.abs(h_gpu[b, c] - h_ref[c])) <= 1e-9 * np.max(np.abs(h_ref[c]))
+    M.mbhl_free(ctx)
+
+
+def test_loglike_parity_config0(table, cfg0):
+    ctx = make_ctx(cfg0)
+    params = cfg0["params"]
+    dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(params))]
+    ll2 = M.mbhl_loglike(ctx, dev(params)).cpu().numpy()
+    assert np.array_equal(ll, ll2)                                  # deterministic reductions
+    pairs, bins = M.mbhl_last_work(ctx)
+    assert 0 < bins <= params.shape[0] * cfg0["freqs"].size and bins <= pairs <= 6 * bins
+    w = L.weights(cfg0["freqs"], cfg0["psd"])
+    dd = L.inner(cfg0["data"], cfg0["data"], w)
+    assert abs(M.mbhl_data_norm(ctx) / dd - 1.0) < 1e-13
+    for b in range(params.shape[0]):
+        rdh, rhh, rll = L.loglike_parts(table, params[b], cfg0["freqs"], cfg0["data"], cfg0["psd"], cfg0["S"], cfg0["t0"])
+        assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (b, ll[b], rll)
+        assert abs(hh[b] - rhh) <= 1e-8 * rhh and abs(dh[b] - rdh) <= 1e-8 * max(abs(rdh), rhh)
+        assert abs(ll[b] - (dh[b] - 0.5 * hh[b] - 0.5 * M.mbhl_data_norm(ctx))) <= 1e-9 * (dd + hh[b])
+    # host-buffer entry point gives the same numbers
+    ph = torch.from_numpy(params.copy()).pin_memory()
+    lh = torch.empty(params.shape[0], dtype=torch.float64).pin_memory()
+    M.mbhl_loglike_host(ctx, ph, lh)
+    assert np.array_equal(lh.numpy(), ll)
+    M.mbhl_free(ctx)
+
+
+def test_noise_free_injection_gives_logl_zero_and_distance_scaling(table):
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    wl = W.build(0, tf, with_noise=False)
+    ctx = make_ctx(wl)
+    inj = wl["injections"][0]
+    p = np.stack([inj, inj, inj])
+    p[1, 4] *= 2.0
+    p[2, 0] *= 1.0 + 1e-5
+    dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(p))]
+    assert abs(ll[0]) < 1e-6 and hh[0] > 1e3
+    assert abs(hh[1] * 4.0 / hh[0] - 1.0) < 1e-12
+    assert ll[2] < -1.0
+    M.mbhl_free(ctx)
+
+
+def test_edge_cases(table, cfg0):
+    # ragged grid (N not a multiple of the chunk or of 32), PSD zeros / non-finite, mode mask, domain errors
+    n = 5 * 512 + 37
+    sl = slice(20000, 20000 + n)
+    freqs = cfg0["freqs"][sl].copy()
+    data = cfg0["data"][:, sl].copy()
+    psd = cfg0["psd"][:, sl].copy()
+    psd[0, 11] = 0.0
+    psd[1, 12] = np.inf
+    psd[2, 13] = np.nan
+    psd[1, 14] = -1.0
+    params = cfg0["params"][:4].copy()
+    bad = params[:3].copy()
+    bad[0, 4] = -5.0           # D_L <= 0
+    bad[1, 2] = 1.5            # |a1| > 1
+    bad[2, 10] = np.nan
+    heavy = params[:1].copy()
+    heavy[0, 0] = 1e10         # every band below the grid
+    allp = np.concatenate([params, bad, heavy])
+    for mask in (0, 0b000001, 0b101010):
+        ctx = M.mbhl_init(dev(freqs), dev(data), dev(psd), sparse_points=64, mode_mask=mask)
+        ll = M.mbhl_loglike(ctx, dev(allp)).cpu().numpy()
+        dd = M.mbhl_data_norm(ctx)
+        w = L.weights(freqs, psd)
+        assert abs(dd / L.inner(data, data, w) - 1.0) < 1e-13
+        assert np.all(np.isneginf(ll[4:7])) and ll[7] == -0.5 * dd and not np.any(np.isnan(ll))
+        for b in range(4):
+            h = L.template(table, allp[b], freqs, 64, 0.0, mode_mask=mask if mask else 0x3F)
+            ref = L.inner(data, h, w) - 0.5 * L.inner(h, h, w) - 0.5 * L.inner(data, data, w)
+            assert abs(ll[b] - ref) <= 1e-6 * (1.0 + abs(ref))
+        # B = 0 is a no-op
+        M.mbhl_loglike(ctx, torch.empty((0, 11), dtype=torch.float64, device=DEV))
+        M.mbhl_free(ctx)
+
+
+def test_host_pointers_at_init_and_workspace_api(table, cfg0):
+    ctx_d = make_ctx(cfg0)
+    ctx_h = M.mbhl_init(cfg0["freqs"], np.ascontiguousarray(cfg0["data"]), np.ascontiguousarray(cfg0["psd"]),
+                        sparse_points=cfg0["S"], t0=cfg0["t0"])
+    p = dev(cfg0["params"])
+    a = M.mbhl_loglike(ctx_d, p).cpu().numpy()
+    b = M.mbhl_loglike(ctx_h, p).cpu().numpy()
+    assert np.array_equal(a, b)
+    need = M.mbhl_workspace_bytes(ctx_h, p.shape[0])
+    assert need > 0
+    ws = torch.empty(need, dtype=torch.uint8, device=DEV)
+    M.mbhl_set_workspace(ctx_h, ws)
+    assert np.array_equal(M.mbhl_loglike(ctx_h, p).cpu().numpy(), a)
+    small = torch.empty(1024, dtype=torch.uint8, device=DEV)
+    M.mbhl_set_workspace(ctx_h, small)
+    with pytest.raises(M.MbhlError, match="workspace"):
+        M.mbhl_loglike(ctx_h, p)
+    M.mbhl_set_workspace(ctx_h, None)
+    assert np.array_equal(M.mbhl_loglike(ctx_h, p).cpu().numpy(), a)
+    assert M.mbhl_launch_count(ctx_h) > 0
+    M.mbhl_free(ctx_d)
+    M.mbhl_free(ctx_h)
+
+
+def test_init_rejects_bad_grids(cfg0):
+    f = cfg0["freqs"][:1000].copy()
+    d = np.ascontiguousarray(cfg0["data"][:, :1000])
+    s = np.ascontiguousarray(cfg0["psd"][:, :1000])
+    bad = f.copy()
+    bad[500] *= 1.001                                  # non-uniform
+    with pytest.raises(M.MbhlError, match="invalid argument"):
+        M.mbhl_init(bad, d, s)
+    with pytest.raises(M.MbhlError, match="invalid argument"):
+        M.mbhl_init(f[::-1].copy(), d, s)              # decreasing
+    with pytest.raises(M.MbhlError, match="invalid argument"):
+        M.mbhl_init(f[:3].copy(), d[:, :3].copy(), s[:, :3].copy())
+    with pytest.raises(M.MbhlError, match="invalid argument"):
+        M.mbhl_init(f, d, s, sparse_points=4)
+
+
+def test_loglike_parity_config1_sampled_walkers(table):
+    # BASELINE config 1 at full size (N = 2^20, S = 512, B = 64): the oracle checks sampled walkers one by one
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    wl = W.build(1, tf)
+    ctx = make_ctx(wl)
+    ll = M.mbhl_loglike(ctx, dev(wl["params"])).cpu().numpy()
+    assert ll.shape == (64,) and np.all(np.isfinite(ll))
+    for b in (0, 17, 63):
+        ref = L.loglike_parts(table, wl["params"][b], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])[2]
+        assert abs(ll[b] - ref) <= 1e-6 * (1.0 + abs(ref)), (b, ll[b], ref)
+    # the injection itself is close to the maximum: logL(injection) ~ -(number of noise dof)/1 + ... >> typical walker
+    inj = M.mbhl_loglike(ctx, dev(wl["injections"])).cpu().numpy()[0]
+    ref = L.loglike_parts(table, wl["injections"][0], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])[2]
+    assert abs(inj - ref) <= 1e-6 * (1.0 + abs(ref))
+    M.mbhl_free(ctx)
