@@ -1,0 +1,281 @@
+#!/usr/bin/env python3
+"""bench.py - log-likelihoods/s of the batched LISA MBHB likelihood hot path on B200 (fp64).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0|1|2] [--impl ours|reference]
+
+A step = one pass of the whole hot path (per-walker constants, PhenomHM + response on the sparse grid,
+spline solve, fused dense interpolation + inner products, final reduction) over one batch of walkers.
+Default workload: BASELINE.json configs[2] (B = 1024 walkers, 6 modes, S = 1024, N = 4 197 160 bins), the
+configuration the north_star's roofline target is quoted on.  N > 1: one process per GPU (torchrun), data
+replicated, walkers sharded - every rank runs its own batch of B walkers, no data-path collective
+("scaling": "weak"); the only communication is the max over ranks of the timings.
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "log-likelihoods/sec"
+FLOP_PER_PAIR = 113.0     # per (walker, bin, active mode)
+FLOP_PER_BIN = 40.0       # per (walker, active bin) epilogue
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x 2 x max SM clock
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def workload_name(cfg, B, N, S):
+    return f"BASELINE.json configs[{cfg}]: B={B} walkers x 6 PhenomHM modes, S={S} sparse knots/mode, N={N} dense bins, A/E/T"
+
+
+def oracle_sample(cfg, n_bins=None):
+    """Builds the workload with the oracle's injections and returns (workload, sample walker indices)."""
+    from oracle import likelihood as L
+    from oracle.constants import load_model_table
+    from paper_2005_01827_b200 import workloads as W
+    table = load_model_table()
+    wl = W.build(cfg, lambda p, f, S: L.template(table, p, f, S), n_bins=n_bins)
+    B = wl["params"].shape[0]
+    idx = [0, B // 2, B - 1] if cfg == 2 else ([0, 1] if cfg == 0 else [0])
+    return table, wl, idx
+
+
+def time_oracle(table, wl, idx):
+    from oracle import likelihood as L
+    t0 = time.perf_counter()
+    for b in idx:
+        L.loglike_parts(table, wl["params"][b], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on this box's host cores (one process, numpy)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    table, wl, idx = oracle_sample(args.config)
+    B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
+    for _ in range(args.warmup):
+        time_oracle(table, wl, idx[:1])
+    t = sum(time_oracle(table, wl, idx) for _ in range(args.steps))
+    value = len(idx) * args.steps / t
+    sample = f"walkers {idx} of the batch per step (one per injection group), full grid, single numpy process"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "logL/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, B, N, S), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "logL/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "logL/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2005_01827_b200 import binding as M
+    from paper_2005_01827_b200 import build as mbuild
+    from paper_2005_01827_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        mbuild.build()
+    if world > 1:
+        dist.barrier()
+    M.lib()
+
+    # ---- workload: grid, PSD, parameters from the seeded generators; injections from the library's own template ----
+    state = {}
+
+    def gpu_template(p, f, S):
+        if "ctx0" not in state:     # a context on a zero data stream, used only to synthesise the injections
+            n = f.size
+            state["ctx0"] = M.mbhl_init(torch.as_tensor(f, device=dev), torch.zeros((3, n, 2), dtype=torch.float64, device=dev),
+                                        torch.ones((3, n), dtype=torch.float64, device=dev), sparse_points=S, device=local)
+        h = M.mbhl_template(state["ctx0"], torch.as_tensor(p[None, :].copy(), device=dev))
+        torch.cuda.synchronize()
+        return h[0].cpu().numpy()
+
+    wl = W.build(args.config, gpu_template)
+    M.mbhl_free(state.pop("ctx0"))
+    B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
+    params_np = wl["params"]
+    if rank > 0:   # each rank gets its own walkers around the same injections (weak scaling)
+        rng = np.random.default_rng(W.SEED0 + 1000 + rank)
+        params_np = params_np * (1.0 + 1e-4 * rng.standard_normal(params_np.shape) * (np.arange(11) == 0))
+    t = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=dev)
+    ctx = M.mbhl_init(t(wl["freqs"]), t(wl["data"]), t(wl["psd"]), sparse_points=S, t0=wl["t0"], max_batch=B, device=local)
+    params = t(params_np)
+    logL = torch.empty(B, dtype=torch.float64, device=dev)
+    params_pin = torch.from_numpy(params_np.copy()).pin_memory()
+    logL_pin = torch.empty(B, dtype=torch.float64).pin_memory()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        v = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        return float(v.item())
+
+    # ---- device-resident timing ----
+    M.mbhl_enable_stage_timing(ctx, True)
+    for _ in range(max(args.warmup, 3)):
+        M.mbhl_loglike(ctx, params, logL)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = M.mbhl_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    M.mbhl_stage_times(ctx)                 # resets the per-call event ring: the mean below covers the timed steps only
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        M.mbhl_loglike(ctx, params, logL)
+    e1.record()
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    launches = M.mbhl_launch_count(ctx) - launches0
+    stage = np.array(M.mbhl_stage_times(ctx)) * args.steps       # mean over the timed steps (CUDA events on the launch stream)
+    pairs, bins = M.mbhl_last_work(ctx)
+    # ---- end to end: host buffers, H2D + D2H inside the timed region ----
+    M.mbhl_loglike_host(ctx, params_pin, logL_pin)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        M.mbhl_loglike_host(ctx, params_pin, logL_pin)     # synchronous: returns after the D2H copy landed
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    clocks = sampler.stop()
+    assert np.array_equal(logL_pin.numpy(), logL.cpu().numpy())
+
+    # ---- FP64 roofline denominator: DFMA-chain probe timed alone, in this run ----
+    sink = torch.zeros(8, dtype=torch.float64, device=dev)
+    blocks, threads, iters = 148 * 8, 256, 20000
+    M.mbhl_dfma_probe(blocks, threads, 200, sink)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    M.mbhl_dfma_probe(blocks, threads, iters, sink)
+    p1.record()
+    torch.cuda.synchronize()
+    fp64_peak = 2.0 * blocks * threads * iters * 8 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    ms_step = ms_total / args.steps
+    value = world * B * args.steps / (ms_total * 1e-3)
+    dense_ms = stage[3] / args.steps
+    flops = FLOP_PER_PAIR * pairs + FLOP_PER_BIN * bins
+    achieved = flops / (dense_ms * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    hbm_bytes = 80.0 * bins          # weighted data + weights + frequency, if nothing were reused across walkers
+    out = {
+        "metric": METRIC, "value": value, "unit": "logL/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config, B, N, S), "walkers_per_gpu": B,
+                   "l2": "inputs larger than L2 (0.34 GB weighted data + 1.6 GB spline coefficients per step vs 126 MB L2)",
+                   "active_pairs_per_step": pairs, "active_bins_per_step": bins,
+                   "stage_ms": {k: float(v / args.steps) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
+        "e2e": {"value": world * B * args.steps / e2e_s, "unit": "logL/s", "h2d_bytes_per_step": int(B * 11 * 8),
+                "d2h_bytes_per_step": int(B * 8)},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "k_dense", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+                     "frac": achieved / fp64_peak, "traffic": None,
+                     "peak_source": "DFMA-chain probe measured in this run (nominal 148 SM x 64 lanes x 2 x 1.965 GHz = %.1f)" % NOMINAL_FP64_TFLOPS,
+                     "algorithmic_flops_per_launch": flops, "dense_ms": dense_ms,
+                     "hbm_bound_ms_if_no_reuse": hbm_bytes / (peaks.get("hbm_gbs", 6650.0) * 1e9) * 1e3},
+    }
+    if args.cpu_baseline:
+        table, owl, idx = oracle_sample(args.config)
+        tcpu = time_oracle(table, owl, idx)
+        out["cpu_baseline"] = {"value": len(idx) / tcpu, "unit": "logL/s", "cores": 1, "kind": "oracle",
+                               "sample": f"walkers {idx} of the batch (one per injection group), full grid, {tcpu:.1f} s"}
+    print(json.dumps(out))
+    M.mbhl_free(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=(0, 1, 2))
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if int(os.environ.get("WORLD_SIZE", "1")) > 1 or args.gpus > 1:
+            args.cpu_baseline = args.cpu_baseline and int(os.environ.get("RANK", "0")) == 0 and int(os.environ.get("WORLD_SIZE", "1")) == 1
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

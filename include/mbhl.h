@@ -121,6 +121,14 @@ int64_t mbhl_launch_count(const mbhl_ctx* ctx);     /* kernels this context has 
  * pairs = sum over walkers and modes of in-band bins, bins = sum over walkers of bins covered by >= 1 mode. */
 int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins);
 
+/* Optional per-stage device timing.  When enabled, mbhl_loglike* records CUDA events on the context's stream
+ * around its five stages; mbhl_stage_times synchronises the stream, returns the MEAN milliseconds per stage
+ * over the calls made since the previous mbhl_stage_times / enable (at most the last 64) and resets the
+ * count: ms[0] per-walker constants, ms[1] sparse evaluation, ms[2] spline solve, ms[3] fused dense kernel,
+ * ms[4] final reduction.  Returns MBHL_EINVAL if timing is off or no call was made.                       */
+int mbhl_enable_stage_timing(mbhl_ctx* ctx, int32_t on);
+int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]);
+
 /* FP64 DFMA-chain probe used to measure the roofline denominator: each of blocks*threads threads runs
  * iters*8 dependent-chain DFMAs (8 independent chains); sink is a device pointer to >= 1 double.
  * Asynchronous on `stream`.  FLOPs = 2 * blocks * threads * iters * 8.                                   */

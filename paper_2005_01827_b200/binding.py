@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
 SYMBOLS = ("mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
-           "mbhl_launch_count", "mbhl_last_work", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
+           "mbhl_launch_count", "mbhl_last_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
 
 
 class mbhl_config(ctypes.Structure):
@@ -56,6 +56,8 @@ def lib():
         L.mbhl_launch_count.argtypes = [vp]
         L.mbhl_launch_count.restype = i64
         L.mbhl_last_work.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        L.mbhl_enable_stage_timing.argtypes = [vp, i32]
+        L.mbhl_stage_times.argtypes = [vp, ctypes.POINTER(dbl * 5)]
         L.mbhl_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
         L.mbhl_strerror.argtypes = [ctypes.c_int]
         L.mbhl_strerror.restype = ctypes.c_char_p
@@ -168,6 +170,17 @@ def mbhl_last_work(ctx):
     p, b = ctypes.c_int64(), ctypes.c_int64()
     _check(lib().mbhl_last_work(ctx, ctypes.byref(p), ctypes.byref(b)), ctx)
     return p.value, b.value
+
+
+def mbhl_enable_stage_timing(ctx, on=True):
+    _check(lib().mbhl_enable_stage_timing(ctx, 1 if on else 0), ctx)
+
+
+def mbhl_stage_times(ctx):
+    """Milliseconds of the last mbhl_loglike* call: (consts, sparse, spline, dense, reduce)."""
+    ms = (ctypes.c_double * 5)()
+    _check(lib().mbhl_stage_times(ctx, ctypes.byref(ms)), ctx)
+    return list(ms)
 
 
 def mbhl_dfma_probe(blocks, threads, iters, sink, stream=None):

@@ -33,6 +33,11 @@ struct mbhl_ctx {
     void* ws_user = nullptr;
     size_t ws_user_bytes = 0;
     int64_t launches = 0;
+    bool timing = false;
+    int n_timed = 0;                       // calls recorded since timing was (re-)enabled
+    static constexpr int kSlots = 64;      // ring of event sets, one per call
+    cudaEvent_t evs[kSlots][6] = {};
+    cudaEvent_t* ev = evs[0];
     char err[512] = {0};
 };
 
@@ -118,11 +123,16 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     double* y = (double*)(base + L.y);
     double* coef = (double*)(base + L.coef);
     const int S = ctx->S;
+    const bool tm = ctx->timing && with_coef;
+    if (tm) ctx->ev = ctx->evs[ctx->n_timed % mbhl_ctx::kSlots];
+    if (tm) cudaEventRecord(ctx->ev[0], ctx->stream);
     k_walker_consts<<<(unsigned)((B + 63) / 64), 64, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
                                                                       ctx->mode_mask, wc);
+    if (tm) cudaEventRecord(ctx->ev[1], ctx->stream);
     dim3 gs((unsigned)(B * MBHL_NMODE), (unsigned)((S + 127) / 128));
     k_sparse_eval<<<gs, 128, 0, ctx->stream>>>(wc, S, knots, y);
     ctx->launches += 2;
+    if (tm) cudaEventRecord(ctx->ev[2], ctx->stream);
     if (with_coef) {
         k_spline<<<(unsigned)(B * MBHL_NMODE), 128, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
         ctx->launches += 1;
@@ -158,6 +168,9 @@ void mbhl_free(mbhl_ctx* ctx) {
     cudaFree(ctx->wdim);
     cudaFree(ctx->counters);
     cudaFree(ctx->ws_internal);
+    for (int k = 0; k < mbhl_ctx::kSlots; ++k)
+        for (int i = 0; i < 6; ++i)
+            if (ctx->evs[k][i]) cudaEventDestroy(ctx->evs[k][i]);
     delete ctx;
 }
 
@@ -315,9 +328,12 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     A.S = ctx->S;
     A.n_chunks = n_chunks_of(ctx->N);
     CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    if (ctx->timing) cudaEventRecord(ctx->ev[3], ctx->stream);
     dim3 gd((unsigned)A.n_chunks, (unsigned)B);
     k_dense<<<gd, kDenseThreads, 0, ctx->stream>>>(A);
+    if (ctx->timing) cudaEventRecord(ctx->ev[4], ctx->stream);
     k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.wc, A.partials, A.n_chunks, B, ctx->dd, d_h, h_h, logL);
+    if (ctx->timing) { cudaEventRecord(ctx->ev[5], ctx->stream); ctx->n_timed += 1; }
     ctx->launches += 2;
     CU(cudaGetLastError());
     return MBHL_OK;
@@ -401,6 +417,33 @@ int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, d
         CU(cudaMemcpyAsync(coef, base + L.coef, (size_t)B * MBHL_NMODE * (ctx->S - 1) * kCoefStride * sizeof(double),
                            cudaMemcpyDeviceToDevice, ctx->stream));
     CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+int mbhl_enable_stage_timing(mbhl_ctx* ctx, int32_t on) {
+    if (!ctx) return MBHL_EINVAL;
+    CU(cudaSetDevice(ctx->device));
+    if (on && !ctx->evs[0][0])
+        for (int k = 0; k < mbhl_ctx::kSlots; ++k)
+            for (int i = 0; i < 6; ++i) CU(cudaEventCreate(&ctx->evs[k][i]));
+    ctx->timing = on != 0;
+    ctx->n_timed = 0;
+    return MBHL_OK;
+}
+
+int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]) {
+    if (!ctx || !ms) return MBHL_EINVAL;
+    if (!ctx->timing || ctx->n_timed == 0) return fail(ctx, MBHL_EINVAL, "stage timing is off or no call was timed");
+    CU(cudaStreamSynchronize(ctx->stream));
+    const int n = ctx->n_timed < mbhl_ctx::kSlots ? ctx->n_timed : mbhl_ctx::kSlots;
+    for (int i = 0; i < 5; ++i) ms[i] = 0.0;
+    for (int k = 0; k < n; ++k)
+        for (int i = 0; i < 5; ++i) {
+            float t = 0.f;
+            CU(cudaEventElapsedTime(&t, ctx->evs[k][i], ctx->evs[k][i + 1]));
+            ms[i] += (double)t / n;
+        }
+    ctx->n_timed = 0;
     return MBHL_OK;
 }
 

@@ -81,17 +81,18 @@ def test_sparse_stage_parity(table, cfg0):
             co = mo["coef"].copy()                    # [S-1, 8, 4]
             co[:, 1, :] /= 2.0 * math.pi
             cg = coef[b, mi]
+            hj = np.diff(mo["knots"])
             for q in range(8):
+                # compare each coefficient through its contribution at the far end of the interval
+                # (c_j h^2 and d_j h^3 are differences of O(y) terms: that is their natural error scale)
+                yscale = 1.0 if q == 1 else (np.max(np.abs(co[:, 0, 0])) if q == 0 else np.max(np.abs(co[:, 2:, 0])))
+                tol = 1e-10 * yscale if q != 1 else 2e-9          # phase: cycles
                 for col in range(4):
-                    ref = co[:, q, col]
-                    got = cg[:, q, col]
+                    d = (cg[:, q, col] - co[:, q, col]) * hj ** col
                     if q == 1 and col == 0:
-                        d = got - ref
-                        assert np.max(np.abs(d - np.rint(d))) <= 1e-8 and np.max(np.abs(got)) <= 0.5 + 1e-12
-                    else:
-                        scale = np.max(np.abs(ref))
-                        if scale > 0:
-                            assert np.max(np.abs(got - ref)) <= 2e-8 * scale, (b, mi, q, col)
+                        d = d - np.rint(d)
+                        assert np.max(np.abs(cg[:, q, col])) <= 0.5 + 1e-12
+                    assert np.max(np.abs(d)) <= tol, (b, mi, q, col, np.max(np.abs(d)), tol)
     M.mbhl_free(ctx)
 
 
@@ -166,7 +167,7 @@ def test_noise_free_injection_gives_logl_zero_and_distance_scaling(table):
     inj = wl["injections"][0]
     p = np.stack([inj, inj, inj])
     p[1, 4] *= 2.0
-    p[2, 0] *= 1.0 + 1e-5
+    p[2, 0] *= 1.0 + 1e-3
     dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(p))]
     assert abs(ll[0]) < 1e-6 and hh[0] > 1e3
     assert abs(hh[1] * 4.0 / hh[0] - 1.0) < 1e-12
