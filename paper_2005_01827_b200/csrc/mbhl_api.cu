@@ -23,9 +23,7 @@ struct mbhl_ctx {
     double f_min = 0.0, f_max = 0.0, df = 0.0, dd = 0.0;
     // library-owned device data
     double* freqs = nullptr;
-    double* w = nullptr;
-    double* wdre = nullptr;
-    double* wdim = nullptr;
+    double* tiles = nullptr;               // [n_chunks][10][512] staged layout of f, w, w d (mbhl_kernels.cuh)
     unsigned long long* counters = nullptr;
     // workspace
     void* ws_internal = nullptr;
@@ -44,8 +42,25 @@ struct mbhl_ctx {
 namespace {
 
 struct WsLayout {
-    size_t params, consts, knots, y, coef, partials, dh, hh, logl, total;
+    size_t params, consts, dense, knots, y, coef, partials, dh, hh, logl, total;
 };
+
+// Launch shape of the fused dense kernel: W walkers per CTA tile, G chunks per CTA.  W amortises the staged
+// data tile (HBM traffic = data bytes x B / W); both shrink for small problems so the grid still fills 148 SMs.
+struct DensePlan {
+    int W, G, n_tiles, n_groups;
+};
+
+DensePlan dense_plan(int64_t B, int n_chunks) {
+    DensePlan p;
+    int64_t w = B * (int64_t)n_chunks / 4096;
+    p.W = (int)(w < 1 ? 1 : (w > kMaxW ? kMaxW : w));
+    p.n_tiles = (int)((B + p.W - 1) / p.W);
+    int64_t g = (int64_t)p.n_tiles * n_chunks / 8192;
+    p.G = (int)(g < 1 ? 1 : (g > 16 ? 16 : g));
+    p.n_groups = (n_chunks + p.G - 1) / p.G;
+    return p;
+}
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -57,10 +72,11 @@ WsLayout layout(const mbhl_ctx* c, int64_t B) {
     const size_t b = (size_t)(B > 0 ? B : 1);
     L.params = off; off += align256(b * MBHL_NPARAM * sizeof(double));
     L.consts = off; off += align256(b * sizeof(WalkerConst));
+    L.dense = off; off += align256(b * sizeof(DenseWalker));
     L.knots = off; off += align256(b * MBHL_NMODE * c->S * sizeof(double));
     L.y = off; off += align256(b * MBHL_NMODE * MBHL_NQ * c->S * sizeof(double));
     L.coef = off; off += align256(b * MBHL_NMODE * (size_t)(c->S - 1) * kCoefStride * sizeof(double));
-    L.partials = off; off += align256(b * (size_t)n_chunks_of(c->N) * 2 * sizeof(double));
+    L.partials = off; off += align256(b * (size_t)dense_plan((int64_t)b, n_chunks_of(c->N)).n_groups * 2 * sizeof(double));
     L.dh = off; off += align256(b * sizeof(double));
     L.hh = off; off += align256(b * sizeof(double));
     L.logl = off; off += align256(b * sizeof(double));
@@ -127,7 +143,8 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     if (tm) ctx->ev = ctx->evs[ctx->n_timed % mbhl_ctx::kSlots];
     if (tm) cudaEventRecord(ctx->ev[0], ctx->stream);
     k_walker_consts<<<(unsigned)((B + 63) / 64), 64, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
-                                                                      ctx->mode_mask, wc);
+                                                                      ctx->mode_mask, ctx->freqs, (int)ctx->N, ctx->df, wc,
+                                                                      (DenseWalker*)(base + L.dense));
     if (tm) cudaEventRecord(ctx->ev[1], ctx->stream);
     dim3 gs((unsigned)(B * MBHL_NMODE), (unsigned)((S + 127) / 128));
     k_sparse_eval<<<gs, 128, 0, ctx->stream>>>(wc, S, knots, y);
@@ -163,9 +180,7 @@ void mbhl_free(mbhl_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->freqs);
-    cudaFree(ctx->w);
-    cudaFree(ctx->wdre);
-    cudaFree(ctx->wdim);
+    cudaFree(ctx->tiles);
     cudaFree(ctx->counters);
     cudaFree(ctx->ws_internal);
     for (int k = 0; k < mbhl_ctx::kSlots; ++k)
@@ -178,7 +193,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
               const mbhl_config* cfg) {
     if (!out) return MBHL_EINVAL;
     *out = nullptr;
-    if (!freqs || !data_AET || !psd_AET || N < 4) return MBHL_EINVAL;
+    if (!freqs || !data_AET || !psd_AET || N < 4 || N > ((int64_t)1 << 31) - 2 * kChunk) return MBHL_EINVAL;
     mbhl_ctx* ctx = new (std::nothrow) mbhl_ctx();
     if (!ctx) return MBHL_ENOMEM;
     if (cfg) {
@@ -197,7 +212,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         cudaFree(d_psd);
         cudaFree(d_part);
         if (code != MBHL_OK) {
-            cudaFree(ctx->freqs); cudaFree(ctx->w); cudaFree(ctx->wdre); cudaFree(ctx->wdim); cudaFree(ctx->counters);
+            cudaFree(ctx->freqs); cudaFree(ctx->tiles); cudaFree(ctx->counters);
             delete ctx;
         }
         return code;
@@ -208,10 +223,12 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
+    if (cudaFuncSetAttribute(k_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileBytes) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
     const size_t nb = (size_t)N * sizeof(double);
-    const int nblk = (int)((N + 1023) / 1024);
-    if (cudaMalloc(&ctx->freqs, nb) != cudaSuccess || cudaMalloc(&ctx->w, 3 * nb) != cudaSuccess ||
-        cudaMalloc(&ctx->wdre, 3 * nb) != cudaSuccess || cudaMalloc(&ctx->wdim, 3 * nb) != cudaSuccess ||
+    const int nblk = (int)((N + 1023) / 1024) > n_chunks_of(N) ? (int)((N + 1023) / 1024) : n_chunks_of(N);
+    if (cudaMalloc(&ctx->freqs, nb) != cudaSuccess ||
+        cudaMalloc(&ctx->tiles, (size_t)n_chunks_of(N) * kTileBytes) != cudaSuccess ||
         cudaMalloc(&ctx->counters, 2 * sizeof(unsigned long long)) != cudaSuccess ||
         cudaMalloc(&d_part, (size_t)nblk * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
@@ -242,16 +259,19 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     ctx->f_max = ends[1];
     ctx->df = (ends[1] - ends[0]) / (double)(N - 1);
     if (!(ctx->f_min > 0.0) || !(ctx->df > 0.0) || !isfinite(ctx->f_max)) return cleanup(MBHL_EINVAL);
-    host_part.resize(nblk);
-    k_check_grid<<<nblk, 256, 0, st>>>(ctx->freqs, N, ctx->df, d_part);
-    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nblk * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+    const int ngrid = (int)((N + 1023) / 1024);
+    host_part.resize(ngrid);
+    k_check_grid<<<ngrid, 256, 0, st>>>(ctx->freqs, N, ctx->df, d_part);
+    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)ngrid * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
-    for (int i = 0; i < nblk; ++i)
+    for (int i = 0; i < ngrid; ++i)
         if (!(host_part[i] <= 1e-6)) return cleanup(MBHL_EINVAL);
-    // weights, weighted data, <d|d>
-    k_init_weights<<<nblk, 256, 0, st>>>(data_dev, psd_dev, N, ctx->df, ctx->w, ctx->wdre, ctx->wdim, d_part);
-    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nblk * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+    // data tiles (weights, weighted data) and <d|d>
+    const int nch = n_chunks_of(N);
+    host_part.resize(nch);
+    k_init_tiles<<<nch, 256, 0, st>>>(ctx->freqs, data_dev, psd_dev, N, ctx->df, ctx->tiles, d_part);
+    if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nch * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
@@ -314,25 +334,26 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     const WsLayout L = layout(ctx, B);
     rc = run_sparse(ctx, params, B, base, L, true);
     if (rc != MBHL_OK) return rc;
+    const DensePlan P = dense_plan(B, n_chunks_of(ctx->N));
     DenseArgs A;
-    A.wc = (const WalkerConst*)(base + L.consts);
+    A.dw = (const DenseWalker*)(base + L.dense);
     A.knots = (const double*)(base + L.knots);
     A.coef = (const double*)(base + L.coef);
-    A.freqs = ctx->freqs;
-    A.w = ctx->w;
-    A.wdre = ctx->wdre;
-    A.wdim = ctx->wdim;
+    A.tiles = ctx->tiles;
     A.partials = (double*)(base + L.partials);
-    A.counters = ctx->counters;
-    A.N = ctx->N;
+    A.B = (int)B;
     A.S = ctx->S;
+    A.W = P.W;
+    A.G = P.G;
     A.n_chunks = n_chunks_of(ctx->N);
+    A.n_groups = P.n_groups;
     CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
     if (ctx->timing) cudaEventRecord(ctx->ev[3], ctx->stream);
-    dim3 gd((unsigned)A.n_chunks, (unsigned)B);
-    k_dense<<<gd, kDenseThreads, 0, ctx->stream>>>(A);
+    dim3 gd((unsigned)P.n_groups, (unsigned)P.n_tiles);
+    k_dense<<<gd, kDenseThreads, kTileBytes, ctx->stream>>>(A);
     if (ctx->timing) cudaEventRecord(ctx->ev[4], ctx->stream);
-    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.wc, A.partials, A.n_chunks, B, ctx->dd, d_h, h_h, logL);
+    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
+                                                                    ctx->counters);
     if (ctx->timing) { cudaEventRecord(ctx->ev[5], ctx->stream); ctx->n_timed += 1; }
     ctx->launches += 2;
     CU(cudaGetLastError());

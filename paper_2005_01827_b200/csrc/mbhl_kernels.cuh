@@ -8,32 +8,45 @@ namespace mbhl {
 
 constexpr int kCoefStride = MBHL_NQ * 4;   // doubles per (walker, mode, interval) record = 256 B
 constexpr int kSplineHalo = 32;            // overlap rows of the block-parallel tridiagonal solve
-constexpr int kDenseThreads = 128;
+constexpr int kDenseThreads = 128;         // 4 warps per CTA
 constexpr int kDenseR = 4;                 // bins per thread per chunk
-constexpr int kChunk = kDenseThreads * kDenseR;
+constexpr int kWarpTile = 32 * kDenseR;    // 128 consecutive bins per warp
+constexpr int kChunk = kDenseThreads * kDenseR;   // 512 bins per CTA step
+constexpr int kTileRows = 10;              // rows of a staged data tile: f, w^{A,E,T}, (w Re d, w Im d)^{A,E,T}
+constexpr int kTileDoubles = kTileRows * kChunk;
+constexpr int kTileBytes = kTileDoubles * 8;      // 40 KB, one bulk copy
+constexpr int kMaxW = 16;                  // walkers per CTA tile (upper bound)
 
 // ---------------------------------------------------------------------------------------------
-// init: weights, weighted data, <d|d>, grid validation
+// init: data tiles (weights, weighted data), <d|d>, grid validation
+// tiles layout [n_chunks][10][512]: row 0 f_k; rows 1-3 w^c = 4 df / S^c; rows 4+2c, 5+2c = w^c Re d^c, w^c Im d^c.
+// Bins k >= N of the last chunk are padding: f continues the grid, every weight is 0.
 // ---------------------------------------------------------------------------------------------
-__global__ void k_init_weights(const double* __restrict__ data, const double* __restrict__ psd, int64_t N, double df,
-                               double* __restrict__ w, double* __restrict__ wdre, double* __restrict__ wdim,
-                               double* __restrict__ dd_part) {
-    // one block handles 1024 consecutive bins of all three channels; fixed-order reduction
+__global__ void __launch_bounds__(256) k_init_tiles(const double* __restrict__ freqs, const double* __restrict__ data,
+                                                    const double* __restrict__ psd, int64_t N, double df,
+                                                    double* __restrict__ tiles, double* __restrict__ dd_part) {
     __shared__ double red[256];
-    const int64_t k0 = (int64_t)blockIdx.x * 1024;
+    const int64_t k0 = (int64_t)blockIdx.x * kChunk;
+    double* tile = tiles + (int64_t)blockIdx.x * kTileDoubles;
     double acc = 0.0;
-    for (int c = 0; c < 3; ++c) {
-        for (int i = threadIdx.x; i < 1024; i += 256) {
-            const int64_t k = k0 + i;
-            if (k < N) {
+    for (int i = threadIdx.x; i < kChunk; i += 256) {
+        const int64_t k = k0 + i;
+        if (k < N) {
+            tile[i] = freqs[k];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
                 const double s = psd[c * N + k];
                 const double ww = (isfinite(s) && s > 0.0) ? 4.0 * df / s : 0.0;
                 const double dre = data[(c * N + k) * 2], dim = data[(c * N + k) * 2 + 1];
-                w[c * N + k] = ww;
-                wdre[c * N + k] = ww * dre;
-                wdim[c * N + k] = ww * dim;
+                tile[(1 + c) * kChunk + i] = ww;
+                tile[(4 + 2 * c) * kChunk + i] = ww * dre;
+                tile[(5 + 2 * c) * kChunk + i] = ww * dim;
                 acc += ww * (dre * dre + dim * dim);
             }
+        } else {
+            tile[i] = freqs[N - 1] + (double)(k - N + 1) * df;
+#pragma unroll
+            for (int r = 1; r < kTileRows; ++r) tile[r * kChunk + i] = 0.0;
         }
     }
     red[threadIdx.x] = acc;
@@ -69,15 +82,69 @@ __global__ void k_check_grid(const double* __restrict__ f, int64_t N, double df,
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1 + a2: per-walker constants and bands (one thread per walker)
+// a1 + a2: per-walker constants and bands (one thread per walker); also the compact DenseWalker record
+// with each band as a bin range of the init grid.
 // ---------------------------------------------------------------------------------------------
+__device__ inline int first_bin_ge(const double* __restrict__ f, int N, double f0, double inv_df, double x) {
+    double e = ceil((x - f0) * inv_df);          // min{k: f_k >= x}, in [0, N]
+    int k = (e < 0.0) ? 0 : ((e > (double)N) ? N : (int)e);
+    while (k > 0 && f[k - 1] >= x) --k;
+    while (k < N && f[k] < x) ++k;
+    return k;
+}
+__device__ inline int last_bin_le(const double* __restrict__ f, int N, double f0, double inv_df, double x) {
+    double e = floor((x - f0) * inv_df) + 1.0;   // max{k: f_k <= x} = min{k: f_k > x} - 1, in [-1, N-1]
+    int k = (e < 0.0) ? 0 : ((e > (double)N) ? N : (int)e);
+    while (k > 0 && f[k - 1] > x) --k;
+    while (k < N && f[k] <= x) ++k;
+    return k - 1;
+}
+
 __global__ void __launch_bounds__(64) k_walker_consts(const double* __restrict__ params, int64_t B, double t0, double f_min,
-                                                      double f_max, int S, uint32_t mode_mask, WalkerConst* __restrict__ out) {
+                                                      double f_max, int S, uint32_t mode_mask, const double* __restrict__ freqs,
+                                                      int N, double df, WalkerConst* __restrict__ out,
+                                                      DenseWalker* __restrict__ dw) {
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     WalkerConst c;
     build_walker(params + b * 11, t0, f_min, f_max, S, mode_mask, c);
     out[b] = c;
+    DenseWalker d;
+    d.t_coal = c.valid ? c.t_coal : 0.0;
+    d.valid = c.valid;
+    d.pad_ = 0;
+    long long pairs = 0;
+    int lo[MBHL_NMODE], hi[MBHL_NMODE];
+    for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+        DenseMode m;
+        m.k_lo = 1; m.k_hi = 0; m.ln_flo = 0.0; m.inv_dlog = 0.0;
+        if (c.valid && c.mode[mi].active) {
+            m.k_lo = first_bin_ge(freqs, N, f_min, 1.0 / df, c.mode[mi].f_lo);
+            m.k_hi = last_bin_le(freqs, N, f_min, 1.0 / df, c.mode[mi].f_hi);
+            m.ln_flo = c.mode[mi].ln_flo;
+            m.inv_dlog = c.mode[mi].inv_dlog;
+            if (m.k_hi >= m.k_lo) pairs += (long long)(m.k_hi - m.k_lo + 1);
+            else { m.k_lo = 1; m.k_hi = 0; }
+        }
+        lo[mi] = m.k_lo; hi[mi] = m.k_hi;
+        d.mode[mi] = m;
+    }
+    // bins covered by at least one mode: length of the union of the six ranges
+    long long bins = 0;
+    int done_to = -1;                               // everything <= done_to is already counted
+    for (int it = 0; it < MBHL_NMODE; ++it) {
+        int best = -1;
+        for (int mi = 0; mi < MBHL_NMODE; ++mi)
+            if (hi[mi] >= lo[mi] && hi[mi] > done_to && (best < 0 || lo[mi] < lo[best])) best = mi;
+        if (best < 0) break;
+        const int a = max(lo[best], done_to + 1);
+        bins += (long long)(hi[best] - a + 1);
+        done_to = hi[best];
+        // ranges fully below done_to are skipped by the hi > done_to test above
+    }
+    d.pairs = pairs;
+    d.bins = bins;
+    dw[b] = d;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -243,36 +310,86 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------------------------
-// a6 + a7: fused dense kernel.  Interpolates every active mode onto the Fourier bins of one chunk,
-// sums the modes per bin, and accumulates <d|h> and <h|h> (eqs. 2, 3, 11); the template
-// is never written to memory.  One CTA per (chunk, walker); thread t owns bins k0 + t + 128 r.
+// a6 + a7: fused dense kernel.  Interpolates every active mode onto the Fourier bins, sums the modes per
+// bin and accumulates <d|h> and <h|h> (eqs. 2, 3, 11); the template is never written to
+// memory.
+//
+// Work decomposition: a CTA owns a tile of W consecutive walkers and a group of G consecutive 512-bin
+// chunks.  For every chunk the 40 KB data tile (f, w, w d) is staged in shared memory by ONE bulk
+// asynchronous copy (TMA, cp.async.bulk + mbarrier) and reused by all W walkers, so HBM sees each data
+// tile once per walker tile instead of once per walker.  A warp owns 128 consecutive bins (lane + 32 r,
+// r < 4).  Per (walker, mode) the warp checks whether its 128 bins lie in one spline interval (the common
+// case above ~1 mHz): then the 256-byte coefficient record is read with warp-uniform 16-byte loads and
+// shared by the 4 bins of every lane; otherwise every bin looks up its own interval.  The loop body is
+// FP64-pipe bound: 8 Horner cubics, the exact linear phase term, a quarter-turn sincos and 3 complex
+// multiply-adds per (bin, mode).
 // ---------------------------------------------------------------------------------------------
 struct DenseArgs {
-    const WalkerConst* wc;
+    const DenseWalker* dw;   // [B]
     const double* knots;     // [B][6][S]
     const double* coef;      // [B][6][S-1][8][4]
-    const double* freqs;     // [N]
-    const double* w;         // [3][N]
-    const double* wdre;      // [3][N]
-    const double* wdim;      // [3][N]
-    double* partials;        // [B][n_chunks][2]
-    unsigned long long* counters;   // [2]: in-band (bin, mode) pairs, bins covered by >= 1 mode
-    int64_t N;
+    const double* tiles;     // [n_chunks][10][512]
+    double* partials;        // [B][n_groups][2]
+    int B;
     int S;
+    int W;                   // walkers per CTA tile (<= kMaxW)
+    int G;                   // chunks per CTA
     int n_chunks;
+    int n_groups;
 };
 
+// sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
+// (Chebyshev-node interpolation in 50-digit arithmetic; max error 2.6e-17 / 1.0e-16 before rounding).
+constexpr double kS0 = 1.5707963267948966, kS1 = -0.6459640975062443, kS2 = 0.07969262624604301,
+                 kS3 = -0.004681754132340976, kS4 = 0.0001604411507421909, kS5 = -3.59864335298231e-06,
+                 kS6 = 5.633933781537854e-08;
+constexpr double kC1 = -1.2337005501361513, kC2 = 0.25366950789986475, kC3 = -0.02086348073494657,
+                 kC4 = 0.000919259950041661, kC5 = -2.520013526428479e-05, kC6 = 4.6552961874867623e-07;
+constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
+
+// sin and cos of p4 quarter turns (angle = p4 pi/2), any |p4| < 2^51.  No conversions, no divides: the
+// nearest integer comes from the magic-number add, the quadrant from the low word of that sum.
+__device__ __forceinline__ void sincos_qturn(double p4, double& sn, double& cs) {
+    const double t = p4 + kRoundMagic;
+    const int n = __double2loint(t);
+    const double y = p4 - (t - kRoundMagic);
+    const double z = y * y;
+    double ps = fma(z, kS6, kS5);
+    double pc = fma(z, kC6, kC5);
+    ps = fma(z, ps, kS4); pc = fma(z, pc, kC4);
+    ps = fma(z, ps, kS3); pc = fma(z, pc, kC3);
+    ps = fma(z, ps, kS2); pc = fma(z, pc, kC2);
+    ps = fma(z, ps, kS1); pc = fma(z, pc, kC1);
+    ps = fma(z, ps, kS0); pc = fma(z, pc, 1.0);
+    ps *= y;
+    const bool odd = (n & 1) != 0;
+    const double a = odd ? pc : ps;      // sin(angle) up to sign
+    const double b = odd ? ps : pc;      // cos(angle) up to sign
+    sn = __hiloint2double(__double2hiint(a) ^ ((n & 2) << 30), __double2loint(a));
+    cs = __hiloint2double(__double2hiint(b) ^ (((n + 1) & 2) << 30), __double2loint(b));
+}
+
+// frac(f * t) in cycles with the product taken exactly (reading G9): f and t are the supplied doubles.
+__device__ __forceinline__ double linear_cycles(double f, double t) {
+    const double p = f * t;
+    const double e = fma(f, t, -p);
+    const double pr = (p + kRoundMagic) - kRoundMagic;
+    return (p - pr) + e;
+}
+
 // Locates the spline interval of frequency f (ln f = lf) on the log-spaced knots x[0..S-1].
-__device__ __forceinline__ int find_interval(const double* __restrict__ x, int S, double f, double lf, const ModeConst& mc) {
-    int j = (int)((lf - mc.ln_flo) * mc.inv_dlog);
+__device__ __forceinline__ int find_interval(const double* __restrict__ x, int S, double f, double lf, double ln_flo,
+                                             double inv_dlog) {
+    int j = (int)((lf - ln_flo) * inv_dlog);
     j = max(0, min(S - 2, j));
     while (j > 0 && f < __ldg(x + j)) --j;
     while (j < S - 2 && f >= __ldg(x + j + 1)) ++j;
     return j;
 }
 
-// One mode's contribution at one bin: 8 Horner cubics, phase in cycles, sincospi, complex MACs.
-__device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, double u, double lin, double h[6]) {
+// One mode's contribution at one bin from the record `rec` (8 cubics in u = f - f_j): used by the
+// per-bin path of the dense kernel and by mbhl_template.  lin4 = 4 frac(f t_coal); amplitude scaled by `gate`.
+__device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, double u, double lin4, double gate, double h[6]) {
     double v[MBHL_NQ];
 #pragma unroll
     for (int q = 0; q < MBHL_NQ; q += 1) {
@@ -280,11 +397,10 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
         const double2 c23 = __ldg(reinterpret_cast<const double2*>(rec + q * 4 + 2));
         v[q] = fma(fma(fma(c23.y, u, c23.x), u, c01.y), u, c01.x);
     }
-    double cyc = v[1] - lin;
-    cyc -= rint(cyc);
     double sn, cs;
-    sincospi(2.0 * cyc, &sn, &cs);
-    const double are = v[0] * cs, aim = v[0] * sn;
+    sincos_qturn(fma(v[1], 4.0, -lin4), sn, cs);
+    const double amp = v[0] * gate;
+    const double are = amp * cs, aim = amp * sn;
     h[0] = fma(are, v[2], fma(-aim, v[3], h[0]));
     h[1] = fma(are, v[3], fma(aim, v[2], h[1]));
     h[2] = fma(are, v[4], fma(-aim, v[5], h[2]));
@@ -293,110 +409,222 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
     h[5] = fma(are, v[7], fma(aim, v[6], h[5]));
 }
 
-// frac(f * t) with the product taken exactly (reading G9): f and t are the supplied doubles.
-__device__ __forceinline__ double linear_cycles(double f, double t) {
-    const double p = f * t;
-    const double e = fma(f, t, -p);
-    return (p - rint(p)) + e;
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
 }
 
-__global__ void __launch_bounds__(kDenseThreads) k_dense(DenseArgs A) {
-    const int chunk = blockIdx.x;
-    const int64_t b = blockIdx.y;
-    const int64_t k0 = (int64_t)chunk * kChunk;
-    const WalkerConst& c = A.wc[b];
-    double* part = A.partials + (b * A.n_chunks + chunk) * 2;
-    // chunk-level early exit: no active mode overlaps [fa, fb]
-    const double fa = A.freqs[k0];
-    const double fb = A.freqs[min(k0 + kChunk, A.N) - 1];
-    bool any = false;
-    if (c.valid) {
-#pragma unroll
-        for (int mi = 0; mi < MBHL_NMODE; ++mi)
-            any = any || (c.mode[mi].active && fb >= c.mode[mi].f_lo && fa <= c.mode[mi].f_hi);
+__global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
+    extern __shared__ __align__(128) double s_tile[];              // [10][512] staged data tile
+    __shared__ DenseWalker s_dw[kMaxW];
+    __shared__ double s_acc[kDenseThreads / 32][kMaxW][2];
+    __shared__ __align__(8) unsigned long long s_bar;
+    __shared__ int s_range[2];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int b0 = blockIdx.y * A.W;
+    const int nb = min(A.W, A.B - b0);
+    // stage the tile's walker records, find the bin range any of them touches
+    if (tid == 0) { s_range[0] = 0x7fffffff; s_range[1] = -1; }
+    for (int i = tid; i < nb * (int)(sizeof(DenseWalker) / 8); i += kDenseThreads)
+        reinterpret_cast<double*>(s_dw)[i] = reinterpret_cast<const double*>(A.dw + b0)[i];
+    for (int i = tid; i < (kDenseThreads / 32) * kMaxW * 2; i += kDenseThreads) (&s_acc[0][0][0])[i] = 0.0;
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s_bar)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (!any) {
-        if (threadIdx.x == 0) { part[0] = 0.0; part[1] = 0.0; }
-        return;
-    }
-    const double t_coal = c.t_coal;
-    double dh = 0.0, hh = 0.0;
-    unsigned int npairs = 0, nbins = 0;
-#pragma unroll 1
-    for (int r = 0; r < kDenseR; ++r) {
-        const int64_t k = k0 + threadIdx.x + r * kDenseThreads;
-        if (k >= A.N) break;
-        const double f = A.freqs[k];
-        const double lf = log(f);
-        const double lin = linear_cycles(f, t_coal);
-        double h[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-        unsigned int hit = 0;
-#pragma unroll 1
-        for (int mi = 0; mi < MBHL_NMODE; ++mi) {
-            const ModeConst& mc = c.mode[mi];
-            if (!mc.active || f < mc.f_lo || f > mc.f_hi) continue;
-            const double* x = A.knots + (b * MBHL_NMODE + mi) * A.S;
-            const int j = find_interval(x, A.S, f, lf, mc);
-            const double u = f - __ldg(x + j);
-            const double* rec = A.coef + ((b * MBHL_NMODE + mi) * (int64_t)(A.S - 1) + j) * kCoefStride;
-            mode_contrib(rec, u, lin, h);
-            ++hit;
-        }
-        if (hit) {
-            npairs += hit;
-            ++nbins;
-#pragma unroll
-            for (int ch = 0; ch < 3; ++ch) {
-                const double wre = A.wdre[ch * A.N + k], wim = A.wdim[ch * A.N + k], ww = A.w[ch * A.N + k];
-                dh = fma(wre, h[2 * ch], fma(wim, h[2 * ch + 1], dh));
-                hh = fma(ww, fma(h[2 * ch], h[2 * ch], h[2 * ch + 1] * h[2 * ch + 1]), hh);
-            }
-        }
-    }
-    // block reduction (fixed order): warp shuffles, then the four warp sums
-    __shared__ double red[2][kDenseThreads / 32];
-    __shared__ unsigned int redc[2][kDenseThreads / 32];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        dh += __shfl_down_sync(0xffffffffu, dh, o);
-        hh += __shfl_down_sync(0xffffffffu, hh, o);
-        npairs += __shfl_down_sync(0xffffffffu, npairs, o);
-        nbins += __shfl_down_sync(0xffffffffu, nbins, o);
-    }
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { red[0][warp] = dh; red[1][warp] = hh; redc[0][warp] = npairs; redc[1][warp] = nbins; }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (tid < nb * MBHL_NMODE) {
+        const DenseWalker& w = s_dw[tid / MBHL_NMODE];
+        const DenseMode& m = w.mode[tid % MBHL_NMODE];
+        if (w.valid && m.k_hi >= m.k_lo) { atomicMin(&s_range[0], m.k_lo); atomicMax(&s_range[1], m.k_hi); }
+    }
+    __syncthreads();
+    const int c_first = max(blockIdx.x * A.G, s_range[0] / kChunk);
+    const int c_last = min(min((int)(blockIdx.x + 1) * A.G, A.n_chunks) - 1, s_range[1] >= 0 ? s_range[1] / kChunk : -1);
+
+    const uint32_t bar = smem_u32(&s_bar);
+    uint32_t parity = 0;
+    for (int chunk = c_first; chunk <= c_last; ++chunk) {
+        __syncthreads();                                            // every reader of the previous tile is done
+        if (tid == 0) {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(kTileBytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(smem_u32(s_tile)), "l"(A.tiles + (int64_t)chunk * kTileDoubles), "r"(kTileBytes), "r"(bar)
+                         : "memory");
+        }
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+
+        const int kt0 = chunk * kChunk + warp * kWarpTile;          // first bin of this warp's 128
+        const double* sf = s_tile + warp * kWarpTile;
+        double f[kDenseR];
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) f[r] = sf[lane + 32 * r];
+        // ln f at the two ends of the warp tile (lane 0 / lane 31 compute, everybody gets both)
+        double lf_mine = log((lane == 0) ? sf[0] : sf[kWarpTile - 1]);
+        const double lf_start = __shfl_sync(0xffffffffu, lf_mine, 0);
+        const double lf_end = __shfl_sync(0xffffffffu, lf_mine, 31);
+
+        for (int wi = 0; wi < nb; ++wi) {
+            const DenseWalker& w = s_dw[wi];
+            if (!w.valid) continue;
+            // lanes 0..5 prepare mode `lane`: in-tile bin range and the spline intervals of its two ends
+            int ja = 0, jb = -1, in_tile = 0;
+            const double* xk = A.knots + ((int64_t)(b0 + wi) * MBHL_NMODE) * A.S;
+            if (lane < MBHL_NMODE) {
+                const DenseMode m = w.mode[lane];
+                const int a = max(kt0, m.k_lo), b = min(kt0 + kWarpTile - 1, m.k_hi);
+                if (a <= b) {
+                    in_tile = 1;
+                    const double* x = xk + lane * A.S;
+                    const double fa = sf[a - kt0], fb = sf[b - kt0];
+                    int j = (a == kt0) ? (int)((lf_start - m.ln_flo) * m.inv_dlog) : 0;
+                    j = max(0, min(A.S - 2, j));
+                    while (j > 0 && fa < __ldg(x + j)) --j;
+                    while (j < A.S - 2 && fa >= __ldg(x + j + 1)) ++j;
+                    ja = j;
+                    j = (b == kt0 + kWarpTile - 1) ? (int)((lf_end - m.ln_flo) * m.inv_dlog) : A.S - 2;
+                    j = max(ja, min(A.S - 2, j));
+                    while (j > ja && fb < __ldg(x + j)) --j;
+                    while (j < A.S - 2 && fb >= __ldg(x + j + 1)) ++j;
+                    jb = j;
+                }
+            }
+            unsigned act = __ballot_sync(0xffffffffu, in_tile) & 0x3Fu;
+            if (!act) continue;
+
+            double lin4[kDenseR], h[kDenseR][6];
+#pragma unroll
+            for (int r = 0; r < kDenseR; ++r) {
+                lin4[r] = 4.0 * linear_cycles(f[r], w.t_coal);
+#pragma unroll
+                for (int i = 0; i < 6; ++i) h[r][i] = 0.0;
+            }
+            while (act) {
+                const int mi = __ffs(act) - 1;
+                act &= act - 1;
+                const int ja_m = __shfl_sync(0xffffffffu, ja, mi), jb_m = __shfl_sync(0xffffffffu, jb, mi);
+                const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
+                const double* x = xk + mi * A.S;
+                const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
+                double gate[kDenseR];
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) {
+                    const int k = kt0 + lane + 32 * r;
+                    gate[r] = (k >= k_lo && k <= k_hi) ? 1.0 : 0.0;
+                }
+                if (ja_m == jb_m) {
+                    // all 128 bins in one interval: warp-uniform coefficient loads shared by the 4 bins per lane
+                    const double* rec = cbase + (int64_t)ja_m * kCoefStride;
+                    const double xj = __ldg(x + ja_m);
+                    double u[kDenseR], are[kDenseR], aim[kDenseR];
+#pragma unroll
+                    for (int r = 0; r < kDenseR; ++r) u[r] = f[r] - xj;
+                    {
+                        const double2 p01 = __ldg(reinterpret_cast<const double2*>(rec + 4));
+                        const double2 p23 = __ldg(reinterpret_cast<const double2*>(rec + 6));
+                        const double2 a01 = __ldg(reinterpret_cast<const double2*>(rec));
+                        const double2 a23 = __ldg(reinterpret_cast<const double2*>(rec + 2));
+#pragma unroll
+                        for (int r = 0; r < kDenseR; ++r) {
+                            const double ph = fma(fma(fma(p23.y, u[r], p23.x), u[r], p01.y), u[r], p01.x);
+                            double sn, cs;
+                            sincos_qturn(fma(ph, 4.0, -lin4[r]), sn, cs);
+                            const double amp = fma(fma(fma(a23.y, u[r], a23.x), u[r], a01.y), u[r], a01.x) * gate[r];
+                            are[r] = amp * cs;
+                            aim[r] = amp * sn;
+                        }
+                    }
+#pragma unroll
+                    for (int ch = 0; ch < 3; ++ch) {
+                        const double2 r01 = __ldg(reinterpret_cast<const double2*>(rec + 8 + 8 * ch));
+                        const double2 r23 = __ldg(reinterpret_cast<const double2*>(rec + 10 + 8 * ch));
+                        const double2 i01 = __ldg(reinterpret_cast<const double2*>(rec + 12 + 8 * ch));
+                        const double2 i23 = __ldg(reinterpret_cast<const double2*>(rec + 14 + 8 * ch));
+#pragma unroll
+                        for (int r = 0; r < kDenseR; ++r) {
+                            const double tre = fma(fma(fma(r23.y, u[r], r23.x), u[r], r01.y), u[r], r01.x);
+                            const double tim = fma(fma(fma(i23.y, u[r], i23.x), u[r], i01.y), u[r], i01.x);
+                            h[r][2 * ch] = fma(are[r], tre, fma(-aim[r], tim, h[r][2 * ch]));
+                            h[r][2 * ch + 1] = fma(are[r], tim, fma(aim[r], tre, h[r][2 * ch + 1]));
+                        }
+                    }
+                } else {
+                    // the warp tile straddles knots: every bin finds its own interval in [ja_m, jb_m]
+#pragma unroll
+                    for (int r = 0; r < kDenseR; ++r) {
+                        if (gate[r] == 0.0) continue;
+                        int j = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
+                        while (j > ja_m && f[r] < __ldg(x + j)) --j;
+                        while (j < jb_m && f[r] >= __ldg(x + j + 1)) ++j;
+                        mode_contrib(cbase + (int64_t)j * kCoefStride, f[r] - __ldg(x + j), lin4[r], 1.0, h[r]);
+                    }
+                }
+            }
+            // inner products of this walker over the warp's 128 bins
+            double dh = 0.0, hh = 0.0;
+#pragma unroll
+            for (int r = 0; r < kDenseR; ++r) {
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) {
+                    const double ww = sf[(1 + ch) * kChunk + lane + 32 * r];
+                    const double wre = sf[(4 + 2 * ch) * kChunk + lane + 32 * r];
+                    const double wim = sf[(5 + 2 * ch) * kChunk + lane + 32 * r];
+                    dh = fma(wre, h[r][2 * ch], fma(wim, h[r][2 * ch + 1], dh));
+                    hh = fma(ww, fma(h[r][2 * ch], h[r][2 * ch], h[r][2 * ch + 1] * h[r][2 * ch + 1]), hh);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                dh += __shfl_down_sync(0xffffffffu, dh, o);
+                hh += __shfl_down_sync(0xffffffffu, hh, o);
+            }
+            if (lane == 0) { s_acc[warp][wi][0] += dh; s_acc[warp][wi][1] += hh; }
+        }
+    }
+    __syncthreads();
+    if (tid < nb) {
         double sdh = 0.0, shh = 0.0;
-        unsigned int sp = 0, sb = 0;
-        for (int i = 0; i < kDenseThreads / 32; ++i) { sdh += red[0][i]; shh += red[1][i]; sp += redc[0][i]; sb += redc[1][i]; }
+#pragma unroll
+        for (int i = 0; i < kDenseThreads / 32; ++i) { sdh += s_acc[i][tid][0]; shh += s_acc[i][tid][1]; }
+        double* part = A.partials + ((int64_t)(b0 + tid) * A.n_groups + blockIdx.x) * 2;
         part[0] = sdh;
         part[1] = shh;
-        if (sp) { atomicAdd(A.counters, (unsigned long long)sp); atomicAdd(A.counters + 1, (unsigned long long)sb); }
     }
 }
 
 // a7: deterministic final reduction, one warp per walker; logL = <d|h> - 1/2<h|h> - 1/2<d|d> (eq. 2)
-__global__ void __launch_bounds__(128) k_final_reduce(const WalkerConst* __restrict__ wc, const double* __restrict__ partials,
-                                                      int n_chunks, int64_t B, double dd, double* __restrict__ d_h,
-                                                      double* __restrict__ h_h, double* __restrict__ logL) {
+__global__ void __launch_bounds__(128) k_final_reduce(const DenseWalker* __restrict__ dw, const double* __restrict__ partials,
+                                                      int n_groups, int64_t B, double dd, double* __restrict__ d_h,
+                                                      double* __restrict__ h_h, double* __restrict__ logL,
+                                                      unsigned long long* __restrict__ counters) {
     const int64_t b = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (b >= B) return;
     const int lane = threadIdx.x & 31;
-    const double* p = partials + b * n_chunks * 2;
+    const double* p = partials + b * n_groups * 2;
     double sdh = 0.0, shh = 0.0;
-    for (int i = lane; i < n_chunks; i += 32) { sdh += p[2 * i]; shh += p[2 * i + 1]; }
+    for (int i = lane; i < n_groups; i += 32) { sdh += p[2 * i]; shh += p[2 * i + 1]; }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         sdh += __shfl_down_sync(0xffffffffu, sdh, o);
         shh += __shfl_down_sync(0xffffffffu, shh, o);
     }
     if (lane == 0) {
-        const bool valid = wc[b].valid != 0;
+        const bool valid = dw[b].valid != 0;
         if (!valid) { sdh = 0.0; shh = 0.0; }
         if (d_h) d_h[b] = sdh;
         if (h_h) h_h[b] = shh;
         if (logL) logL[b] = valid ? (sdh - 0.5 * shh - 0.5 * dd) : -INFINITY;
+        if (valid && dw[b].pairs) {
+            atomicAdd(counters, (unsigned long long)dw[b].pairs);
+            atomicAdd(counters + 1, (unsigned long long)dw[b].bins);
+        }
     }
 }
 
@@ -415,17 +643,15 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
     if (c.valid) {
         const double f = freqs[k];
         const double lf = log(f);
-        const double lin = linear_cycles(f, c.t_coal);
+        const double lin4 = 4.0 * linear_cycles(f, c.t_coal);
         for (int mi = 0; mi < MBHL_NMODE; ++mi) {
             const ModeConst& mc = c.mode[mi];
             if (!mc.active || !(f >= mc.f_lo) || !(f <= mc.f_hi)) continue;
             if (direct) {
                 double q[MBHL_NQ];
                 smooth_quantities(c, mi, f, q);
-                double cyc = q[1] - rint(q[1]) - lin;
-                cyc -= rint(cyc);
                 double sn, cs;
-                sincospi(2.0 * cyc, &sn, &cs);
+                sincos_qturn(fma(q[1] - rint(q[1]), 4.0, -lin4), sn, cs);
                 const double are = q[0] * cs, aim = q[0] * sn;
                 h[0] += are * q[2] - aim * q[3];
                 h[1] += are * q[3] + aim * q[2];
@@ -435,9 +661,9 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
                 h[5] += are * q[7] + aim * q[6];
             } else {
                 const double* x = knots + (b * MBHL_NMODE + mi) * S;
-                const int j = find_interval(x, S, f, lf, mc);
+                const int j = find_interval(x, S, f, lf, mc.ln_flo, mc.inv_dlog);
                 const double u = f - x[j];
-                mode_contrib(coef + ((b * MBHL_NMODE + mi) * (int64_t)(S - 1) + j) * kCoefStride, u, lin, h);
+                mode_contrib(coef + ((b * MBHL_NMODE + mi) * (int64_t)(S - 1) + j) * kCoefStride, u, lin4, 1.0, h);
             }
         }
     }

@@ -78,6 +78,22 @@ struct WalkerConst {
     ModeConst mode[MBHL_NMODE];
 };
 
+// Compact per-walker record read by the fused dense kernel (step a6/a7): the bin range of every mode's band
+// on the init grid (k_lo = min{k: f_k >= f_lo}, k_hi = max{k: f_k <= f_hi}; empty: k_lo > k_hi) and the
+// constants of the log-spaced knot grid used to guess a bin's spline interval.
+struct DenseMode {
+    int k_lo, k_hi;
+    double ln_flo, inv_dlog;
+};
+struct DenseWalker {
+    double t_coal;
+    int valid;
+    int pad_;
+    long long pairs;            // sum over modes of in-band bins
+    long long bins;             // bins covered by at least one mode
+    DenseMode mode[MBHL_NMODE];
+};
+
 // ---------------------------------------------------------------------------------------------
 // PhenomD pieces (all frequencies are Mf)
 // ---------------------------------------------------------------------------------------------
