@@ -223,7 +223,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
-    if (cudaFuncSetAttribute(k_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileBytes) != cudaSuccess)
+    if (cudaFuncSetAttribute(k_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, kDenseSmemBytes) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
     const size_t nb = (size_t)N * sizeof(double);
     const int nblk = (int)((N + 1023) / 1024) > n_chunks_of(N) ? (int)((N + 1023) / 1024) : n_chunks_of(N);
@@ -349,8 +349,7 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     A.n_groups = P.n_groups;
     CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
     if (ctx->timing) cudaEventRecord(ctx->ev[3], ctx->stream);
-    dim3 gd((unsigned)P.n_groups, (unsigned)P.n_tiles);
-    k_dense<<<gd, kDenseThreads, kTileBytes, ctx->stream>>>(A);
+    k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);
     if (ctx->timing) cudaEventRecord(ctx->ev[4], ctx->stream);
     k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
                                                                     ctx->counters);

@@ -15,7 +15,8 @@ constexpr int kChunk = kDenseThreads * kDenseR;   // 512 bins per CTA step
 constexpr int kTileRows = 10;              // rows of a staged data tile: f, w^{A,E,T}, (w Re d, w Im d)^{A,E,T}
 constexpr int kTileDoubles = kTileRows * kChunk;
 constexpr int kTileBytes = kTileDoubles * 8;      // 40 KB, one bulk copy
-constexpr int kMaxW = 16;                  // walkers per CTA tile (upper bound)
+constexpr int kMaxW = 8;                   // walkers per CTA tile (upper bound)
+constexpr int kPairs = kMaxW * MBHL_NMODE; // (walker, mode) pairs of a CTA tile: one staged coefficient record each
 
 // ---------------------------------------------------------------------------------------------
 // init: data tiles (weights, weighted data), <d|d>, grid validation
@@ -409,195 +410,11 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
     h[5] = fma(are, v[7], fma(aim, v[6], h[5]));
 }
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+}  // namespace mbhl
 
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    } while (!ok);
-}
+#include "mbhl_dense.cuh"   // a6 + a7: the fused dense kernel
 
-__global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
-    extern __shared__ __align__(128) double s_tile[];              // [10][512] staged data tile
-    __shared__ DenseWalker s_dw[kMaxW];
-    __shared__ double s_acc[kDenseThreads / 32][kMaxW][2];
-    __shared__ __align__(8) unsigned long long s_bar;
-    __shared__ int s_range[2];
-
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int b0 = blockIdx.y * A.W;
-    const int nb = min(A.W, A.B - b0);
-    // stage the tile's walker records, find the bin range any of them touches
-    if (tid == 0) { s_range[0] = 0x7fffffff; s_range[1] = -1; }
-    for (int i = tid; i < nb * (int)(sizeof(DenseWalker) / 8); i += kDenseThreads)
-        reinterpret_cast<double*>(s_dw)[i] = reinterpret_cast<const double*>(A.dw + b0)[i];
-    for (int i = tid; i < (kDenseThreads / 32) * kMaxW * 2; i += kDenseThreads) (&s_acc[0][0][0])[i] = 0.0;
-    if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s_bar)) : "memory");
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (tid < nb * MBHL_NMODE) {
-        const DenseWalker& w = s_dw[tid / MBHL_NMODE];
-        const DenseMode& m = w.mode[tid % MBHL_NMODE];
-        if (w.valid && m.k_hi >= m.k_lo) { atomicMin(&s_range[0], m.k_lo); atomicMax(&s_range[1], m.k_hi); }
-    }
-    __syncthreads();
-    const int c_first = max(blockIdx.x * A.G, s_range[0] / kChunk);
-    const int c_last = min(min((int)(blockIdx.x + 1) * A.G, A.n_chunks) - 1, s_range[1] >= 0 ? s_range[1] / kChunk : -1);
-
-    const uint32_t bar = smem_u32(&s_bar);
-    uint32_t parity = 0;
-    for (int chunk = c_first; chunk <= c_last; ++chunk) {
-        __syncthreads();                                            // every reader of the previous tile is done
-        if (tid == 0) {
-            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(kTileBytes) : "memory");
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                         ::"r"(smem_u32(s_tile)), "l"(A.tiles + (int64_t)chunk * kTileDoubles), "r"(kTileBytes), "r"(bar)
-                         : "memory");
-        }
-        mbar_wait(bar, parity);
-        parity ^= 1u;
-
-        const int kt0 = chunk * kChunk + warp * kWarpTile;          // first bin of this warp's 128
-        const double* sf = s_tile + warp * kWarpTile;
-        double f[kDenseR];
-#pragma unroll
-        for (int r = 0; r < kDenseR; ++r) f[r] = sf[lane + 32 * r];
-        // ln f at the two ends of the warp tile (lane 0 / lane 31 compute, everybody gets both)
-        double lf_mine = log((lane == 0) ? sf[0] : sf[kWarpTile - 1]);
-        const double lf_start = __shfl_sync(0xffffffffu, lf_mine, 0);
-        const double lf_end = __shfl_sync(0xffffffffu, lf_mine, 31);
-
-        for (int wi = 0; wi < nb; ++wi) {
-            const DenseWalker& w = s_dw[wi];
-            if (!w.valid) continue;
-            // lanes 0..5 prepare mode `lane`: in-tile bin range and the spline intervals of its two ends
-            int ja = 0, jb = -1, in_tile = 0;
-            const double* xk = A.knots + ((int64_t)(b0 + wi) * MBHL_NMODE) * A.S;
-            if (lane < MBHL_NMODE) {
-                const DenseMode m = w.mode[lane];
-                const int a = max(kt0, m.k_lo), b = min(kt0 + kWarpTile - 1, m.k_hi);
-                if (a <= b) {
-                    in_tile = 1;
-                    const double* x = xk + lane * A.S;
-                    const double fa = sf[a - kt0], fb = sf[b - kt0];
-                    int j = (a == kt0) ? (int)((lf_start - m.ln_flo) * m.inv_dlog) : 0;
-                    j = max(0, min(A.S - 2, j));
-                    while (j > 0 && fa < __ldg(x + j)) --j;
-                    while (j < A.S - 2 && fa >= __ldg(x + j + 1)) ++j;
-                    ja = j;
-                    j = (b == kt0 + kWarpTile - 1) ? (int)((lf_end - m.ln_flo) * m.inv_dlog) : A.S - 2;
-                    j = max(ja, min(A.S - 2, j));
-                    while (j > ja && fb < __ldg(x + j)) --j;
-                    while (j < A.S - 2 && fb >= __ldg(x + j + 1)) ++j;
-                    jb = j;
-                }
-            }
-            unsigned act = __ballot_sync(0xffffffffu, in_tile) & 0x3Fu;
-            if (!act) continue;
-
-            double lin4[kDenseR], h[kDenseR][6];
-#pragma unroll
-            for (int r = 0; r < kDenseR; ++r) {
-                lin4[r] = 4.0 * linear_cycles(f[r], w.t_coal);
-#pragma unroll
-                for (int i = 0; i < 6; ++i) h[r][i] = 0.0;
-            }
-            while (act) {
-                const int mi = __ffs(act) - 1;
-                act &= act - 1;
-                const int ja_m = __shfl_sync(0xffffffffu, ja, mi), jb_m = __shfl_sync(0xffffffffu, jb, mi);
-                const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
-                const double* x = xk + mi * A.S;
-                const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
-                double gate[kDenseR];
-#pragma unroll
-                for (int r = 0; r < kDenseR; ++r) {
-                    const int k = kt0 + lane + 32 * r;
-                    gate[r] = (k >= k_lo && k <= k_hi) ? 1.0 : 0.0;
-                }
-                if (ja_m == jb_m) {
-                    // all 128 bins in one interval: warp-uniform coefficient loads shared by the 4 bins per lane
-                    const double* rec = cbase + (int64_t)ja_m * kCoefStride;
-                    const double xj = __ldg(x + ja_m);
-                    double u[kDenseR], are[kDenseR], aim[kDenseR];
-#pragma unroll
-                    for (int r = 0; r < kDenseR; ++r) u[r] = f[r] - xj;
-                    {
-                        const double2 p01 = __ldg(reinterpret_cast<const double2*>(rec + 4));
-                        const double2 p23 = __ldg(reinterpret_cast<const double2*>(rec + 6));
-                        const double2 a01 = __ldg(reinterpret_cast<const double2*>(rec));
-                        const double2 a23 = __ldg(reinterpret_cast<const double2*>(rec + 2));
-#pragma unroll
-                        for (int r = 0; r < kDenseR; ++r) {
-                            const double ph = fma(fma(fma(p23.y, u[r], p23.x), u[r], p01.y), u[r], p01.x);
-                            double sn, cs;
-                            sincos_qturn(fma(ph, 4.0, -lin4[r]), sn, cs);
-                            const double amp = fma(fma(fma(a23.y, u[r], a23.x), u[r], a01.y), u[r], a01.x) * gate[r];
-                            are[r] = amp * cs;
-                            aim[r] = amp * sn;
-                        }
-                    }
-#pragma unroll
-                    for (int ch = 0; ch < 3; ++ch) {
-                        const double2 r01 = __ldg(reinterpret_cast<const double2*>(rec + 8 + 8 * ch));
-                        const double2 r23 = __ldg(reinterpret_cast<const double2*>(rec + 10 + 8 * ch));
-                        const double2 i01 = __ldg(reinterpret_cast<const double2*>(rec + 12 + 8 * ch));
-                        const double2 i23 = __ldg(reinterpret_cast<const double2*>(rec + 14 + 8 * ch));
-#pragma unroll
-                        for (int r = 0; r < kDenseR; ++r) {
-                            const double tre = fma(fma(fma(r23.y, u[r], r23.x), u[r], r01.y), u[r], r01.x);
-                            const double tim = fma(fma(fma(i23.y, u[r], i23.x), u[r], i01.y), u[r], i01.x);
-                            h[r][2 * ch] = fma(are[r], tre, fma(-aim[r], tim, h[r][2 * ch]));
-                            h[r][2 * ch + 1] = fma(are[r], tim, fma(aim[r], tre, h[r][2 * ch + 1]));
-                        }
-                    }
-                } else {
-                    // the warp tile straddles knots: every bin finds its own interval in [ja_m, jb_m]
-#pragma unroll
-                    for (int r = 0; r < kDenseR; ++r) {
-                        if (gate[r] == 0.0) continue;
-                        int j = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
-                        while (j > ja_m && f[r] < __ldg(x + j)) --j;
-                        while (j < jb_m && f[r] >= __ldg(x + j + 1)) ++j;
-                        mode_contrib(cbase + (int64_t)j * kCoefStride, f[r] - __ldg(x + j), lin4[r], 1.0, h[r]);
-                    }
-                }
-            }
-            // inner products of this walker over the warp's 128 bins
-            double dh = 0.0, hh = 0.0;
-#pragma unroll
-            for (int r = 0; r < kDenseR; ++r) {
-#pragma unroll
-                for (int ch = 0; ch < 3; ++ch) {
-                    const double ww = sf[(1 + ch) * kChunk + lane + 32 * r];
-                    const double wre = sf[(4 + 2 * ch) * kChunk + lane + 32 * r];
-                    const double wim = sf[(5 + 2 * ch) * kChunk + lane + 32 * r];
-                    dh = fma(wre, h[r][2 * ch], fma(wim, h[r][2 * ch + 1], dh));
-                    hh = fma(ww, fma(h[r][2 * ch], h[r][2 * ch], h[r][2 * ch + 1] * h[r][2 * ch + 1]), hh);
-                }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                dh += __shfl_down_sync(0xffffffffu, dh, o);
-                hh += __shfl_down_sync(0xffffffffu, hh, o);
-            }
-            if (lane == 0) { s_acc[warp][wi][0] += dh; s_acc[warp][wi][1] += hh; }
-        }
-    }
-    __syncthreads();
-    if (tid < nb) {
-        double sdh = 0.0, shh = 0.0;
-#pragma unroll
-        for (int i = 0; i < kDenseThreads / 32; ++i) { sdh += s_acc[i][tid][0]; shh += s_acc[i][tid][1]; }
-        double* part = A.partials + ((int64_t)(b0 + tid) * A.n_groups + blockIdx.x) * 2;
-        part[0] = sdh;
-        part[1] = shh;
-    }
-}
+namespace mbhl {
 
 // a7: deterministic final reduction, one warp per walker; logL = <d|h> - 1/2<h|h> - 1/2<d|d> (eq. 2)
 __global__ void __launch_bounds__(128) k_final_reduce(const DenseWalker* __restrict__ dw, const double* __restrict__ partials,
