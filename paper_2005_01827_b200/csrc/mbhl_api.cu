@@ -347,6 +347,7 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     A.G = P.G;
     A.n_chunks = n_chunks_of(ctx->N);
     A.n_groups = P.n_groups;
+    A.inv_df = 1.0 / ctx->df;
     CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
     if (ctx->timing) cudaEventRecord(ctx->ev[3], ctx->stream);
     k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);

@@ -84,8 +84,11 @@ __device__ __forceinline__ void sincos_qturn_x(const double (&p4)[kDenseR], doub
 
 // One mode's contribution to the kDenseR bins of a lane when all of them lie in one spline interval and in
 // band: `rec` is that interval's record (shared or global memory, same address for every lane), xj its knot.
+// kGated: the amplitude of bin r is multiplied by gate[r] (1 inside the segment served by `rec`, else 0).
+template <bool kGated>
 __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, double xj, const double (&f)[kDenseR],
-                                             const double (&lin4)[kDenseR], double (&h)[kDenseR][6]) {
+                                             const double (&lin4)[kDenseR], const double (&gate)[kDenseR],
+                                             double (&h)[kDenseR][6]) {
     double u[kDenseR], are[kDenseR], aim[kDenseR];
 #pragma unroll
     for (int r = 0; r < kDenseR; ++r) u[r] = f[r] - xj;
@@ -111,6 +114,10 @@ __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, dou
         for (int r = 0; r < kDenseR; ++r) amp[r] = fma(amp[r], u[r], a01.y);
 #pragma unroll
         for (int r = 0; r < kDenseR; ++r) amp[r] = fma(amp[r], u[r], a01.x);
+        if (kGated) {
+#pragma unroll
+            for (int r = 0; r < kDenseR; ++r) amp[r] *= gate[r];
+        }
 #pragma unroll
         for (int r = 0; r < kDenseR; ++r) { are[r] = amp[r] * cs[r]; aim[r] = amp[r] * sn[r]; }
     }
@@ -135,17 +142,30 @@ __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, dou
     }
 }
 
-constexpr int kDenseSmemBytes = kTileBytes + kPairs * kCoefStride * (int)sizeof(double);   // 40 KB tile + 12 KB records
+// What the prepare step found for one (walker, mode) pair in the current chunk; offsets are bins within the chunk.
+struct PairDesc {
+    short a, b;      // in-band bins [a, b]
+    short ks;        // first bin of the second staged interval (b + 1 when the pair stays in one interval)
+    short kind;      // 0: no in-band bin, 1: one or two staged records (slots 2p, 2p+1), 2: three or more intervals
+};
+
+constexpr int kRecSlots = 2 * kPairs;                                                       // two records per pair
+constexpr int kDenseSmemBytes = kTileBytes + kRecSlots * kCoefStride * (int)sizeof(double);   // 40 KB tile + 24 KB records
+
+__device__ __forceinline__ void stage_record(double* dst, const double* __restrict__ src) {
+#pragma unroll
+    for (int i = 0; i < kCoefStride; i += 2) cp_async16(dst + i, src + i);
+}
 
 // Grid: 1-D, block id = group * n_tiles + tile (walker tiles vary fastest, so the CTAs resident at one time
 // share a few chunk groups and the data tiles are served by L2).
-__global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
+__global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseArgs A) {
     extern __shared__ __align__(128) double s_dyn[];
     double* const s_tile = s_dyn;                                   // [10][512] staged data tile
-    double* const s_rec = s_dyn + kTileDoubles;                     // [kPairs][32] staged coefficient records
+    double* const s_rec = s_dyn + kTileDoubles;                     // [kRecSlots][32] staged coefficient records
     __shared__ DenseWalker s_dw[kMaxW];
-    __shared__ double s_xj[kPairs];                                 // knot x_j of the staged record
-    __shared__ unsigned s_desc[kPairs];                             // 2 bits per warp: 0 none, 1 fast, 2 general
+    __shared__ double s_xj[kRecSlots];                              // knot x_j of each staged record
+    __shared__ PairDesc s_desc[kPairs];
     __shared__ double s_acc[kDenseThreads / 32][kMaxW][2];
     __shared__ __align__(8) unsigned long long s_bar;
     __shared__ int s_range[2];
@@ -174,8 +194,11 @@ __global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
     if (p_m.k_hi >= p_m.k_lo) { atomicMin(&s_range[0], p_m.k_lo); atomicMax(&s_range[1], p_m.k_hi); }
     const double* const p_x = A.knots + ((int64_t)(b0 + p_wi) * MBHL_NMODE + p_mi) * A.S;
     const double* const p_coef = A.coef + ((int64_t)(b0 + p_wi) * MBHL_NMODE + p_mi) * (int64_t)(A.S - 1) * kCoefStride;
-    int c_j = -1;                                                   // interval whose record is staged in s_rec[tid]
-    double c_lo = 0.0, c_hi = 0.0;                                  // it serves f in [c_lo, c_hi)
+    // staged intervals, kept in registers across chunks: slot 2p holds interval c_j, serving f in [c_lo, c_hi);
+    // slot 2p+1 holds interval c_j + 1 when c_b is set, serving [c_hi, c_hi2)
+    int c_j = -1;
+    bool c_b = false;
+    double c_lo = 0.0, c_hi = 0.0, c_hi2 = 0.0;
     __syncthreads();
     const int c_first = max(group * A.G, s_range[0] / kChunk);
     const int c_last = min(min((group + 1) * A.G, A.n_chunks) - 1, s_range[1] >= 0 ? s_range[1] / kChunk : -1);
@@ -196,52 +219,80 @@ __global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
         // ---- prepare: one thread per (walker, mode) pair ----
         const int kc0 = chunk * kChunk;
         if (p_own) {
-            unsigned desc = 0;
-            const int a = max(kc0, p_m.k_lo), b = min(kc0 + kChunk - 1, p_m.k_hi);
+            PairDesc d;
+            d.a = 0; d.b = -1; d.ks = 0; d.kind = 0;
+            const int a = max(kc0, p_m.k_lo) - kc0, b = min(kc0 + kChunk - 1, p_m.k_hi) - kc0;
             if (a <= b) {
-                const double fa = s_tile[a - kc0], fb = s_tile[b - kc0];
-                bool uni = c_j >= 0 && fa >= c_lo && fb < c_hi;
-                if (!uni) {
-                    const int j = find_interval(p_x, A.S, fa, log(fa), p_m.ln_flo, p_m.inv_dlog);
-                    const double xlo = __ldg(p_x + j), xhi = __ldg(p_x + j + 1);
-                    if (fb < xhi || j == A.S - 2) {
-                        uni = true;
-                        c_j = j;
-                        c_lo = (j == 0) ? -1.0 : xlo;
-                        c_hi = (j == A.S - 2) ? 1e300 : xhi;
-                        s_xj[tid] = xlo;
-                        const double* src = p_coef + (int64_t)j * kCoefStride;
-                        double* dst = s_rec + tid * kCoefStride;
-#pragma unroll
-                        for (int i = 0; i < kCoefStride; i += 2) cp_async16(dst + i, src + i);
-                    } else {
-                        c_j = -1;
-                    }
+                const double fa = s_tile[a], fb = s_tile[b];
+                if (!(c_j >= 0 && fa >= c_lo && fa < c_hi)) {
+                    // the first in-band bin left the staged interval: usually into the next one
+                    int j;
+                    if (c_j >= 0 && fa >= c_hi && fa < c_hi2) j = c_j + 1;
+                    else j = find_interval(p_x, A.S, fa, log(fa), p_m.ln_flo, p_m.inv_dlog);
+                    c_j = j;
+                    c_b = false;
+                    const double xlo = __ldg(p_x + j);
+                    c_lo = (j == 0) ? -1.0 : xlo;
+                    c_hi = (j >= A.S - 2) ? 1e300 : __ldg(p_x + j + 1);
+                    c_hi2 = (j >= A.S - 3) ? 1e300 : __ldg(p_x + j + 2);
+                    s_xj[2 * tid] = xlo;
+                    stage_record(s_rec + (2 * tid) * kCoefStride, p_coef + (int64_t)j * kCoefStride);
                 }
-#pragma unroll
-                for (int w4 = 0; w4 < kDenseThreads / 32; ++w4) {
-                    const int t0 = kc0 + w4 * kWarpTile, t1 = t0 + kWarpTile - 1;
-                    const unsigned kind = (t1 < a || t0 > b) ? 0u : ((uni && t0 >= a && t1 <= b) ? 1u : 2u);
-                    desc |= kind << (2 * w4);
+                d.a = (short)a; d.b = (short)b;
+                if (fb < c_hi) {
+                    d.ks = (short)(b + 1);
+                    d.kind = 1;
+                } else if (fb < c_hi2) {
+                    if (!c_b) {
+                        c_b = true;
+                        s_xj[2 * tid + 1] = c_hi;
+                        stage_record(s_rec + (2 * tid + 1) * kCoefStride, p_coef + (int64_t)(c_j + 1) * kCoefStride);
+                    }
+                    // first bin with f >= c_hi: fa < c_hi <= fb, so it lies in (a, b]
+                    int i = a + (int)ceil((c_hi - fa) * A.inv_df);
+                    i = max(a + 1, min(b, i));
+                    while (i > a + 1 && s_tile[i - 1] >= c_hi) --i;
+                    while (i < b && s_tile[i] < c_hi) ++i;
+                    d.ks = (short)i;
+                    d.kind = 1;
+                } else {
+                    d.kind = 2;
                 }
             }
-            s_desc[tid] = desc;
+            s_desc[tid] = d;
         }
         cp_async_wait_all();
         __syncthreads();
 
         // ---- evaluate: every warp loops over the walkers of the tile ----
-        const int kt0 = kc0 + warp * kWarpTile;                     // first bin of this warp's 128
-        const double* sf = s_tile + warp * kWarpTile;
+        const int t0 = warp * kWarpTile, t1 = t0 + kWarpTile - 1;   // this warp's bins, as offsets in the chunk
+        const int kt0 = kc0 + t0;
+        const double* sf = s_tile + t0;
         double f[kDenseR];
 #pragma unroll
         for (int r = 0; r < kDenseR; ++r) f[r] = sf[lane + 32 * r];
 
         for (int wi = 0; wi < nb; ++wi) {
-            const unsigned kind = (lane < MBHL_NMODE) ? ((s_desc[wi * MBHL_NMODE + lane] >> (2 * warp)) & 3u) : 0u;
-            unsigned m_fast = __ballot_sync(0xffffffffu, kind == 1u);
-            unsigned m_gen = __ballot_sync(0xffffffffu, kind == 2u);
-            if (!(m_fast | m_gen)) continue;
+            // lanes 0..5 classify mode `lane` for this warp tile: segment A = bins served by slot 2p, B = by slot 2p+1
+            int loA = 1, hiA = 0, loB = 1, hiB = 0;
+            bool fullA = false, fullB = false, part = false, gen = false;
+            if (lane < MBHL_NMODE) {
+                const PairDesc d = s_desc[wi * MBHL_NMODE + lane];
+                if (d.kind == 1) {
+                    loA = max((int)d.a, t0); hiA = min((int)d.ks - 1, t1);
+                    loB = max((int)d.ks, t0); hiB = min((int)d.b, t1);
+                    fullA = loA == t0 && hiA == t1;
+                    fullB = loB == t0 && hiB == t1;
+                    part = !fullA && !fullB && (loA <= hiA || loB <= hiB);
+                } else if (d.kind == 2) {
+                    gen = max((int)d.a, t0) <= min((int)d.b, t1);
+                }
+            }
+            unsigned m_full = __ballot_sync(0xffffffffu, fullA || fullB);
+            const unsigned m_selB = __ballot_sync(0xffffffffu, fullB);
+            unsigned m_part = __ballot_sync(0xffffffffu, part);
+            unsigned m_gen = __ballot_sync(0xffffffffu, gen);
+            if (!(m_full | m_part | m_gen)) continue;
             const double t_coal = s_dw[wi].t_coal;
 
             double lin4[kDenseR], h[kDenseR][6];
@@ -251,19 +302,39 @@ __global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
 #pragma unroll
                 for (int i = 0; i < 6; ++i) h[r][i] = 0.0;
             }
-            while (m_fast) {
-                const int mi = __ffs(m_fast) - 1;
-                m_fast &= m_fast - 1;
-                const int p = wi * MBHL_NMODE + mi;
-                mode_uniform(s_rec + p * kCoefStride, s_xj[p], f, lin4, h);
+            while (m_full) {
+                const int mi = __ffs(m_full) - 1;
+                m_full &= m_full - 1;
+                const int slot = 2 * (wi * MBHL_NMODE + mi) + ((m_selB >> mi) & 1u);
+                mode_uniform<false>(s_rec + slot * kCoefStride, s_xj[slot], f, lin4, lin4, h);
+            }
+            while (m_part) {
+                // band edge or knot inside the warp tile: each staged segment is evaluated on all bins and gated
+                const int mi = __ffs(m_part) - 1;
+                m_part &= m_part - 1;
+                const int lo0 = __shfl_sync(0xffffffffu, loA, mi), hi0 = __shfl_sync(0xffffffffu, hiA, mi);
+                const int lo1 = __shfl_sync(0xffffffffu, loB, mi), hi1 = __shfl_sync(0xffffffffu, hiB, mi);
+#pragma unroll 1
+                for (int seg = 0; seg < 2; ++seg) {
+                    const int lo = seg ? lo1 : lo0, hi = seg ? hi1 : hi0;
+                    if (lo > hi) continue;
+                    double gate[kDenseR];
+#pragma unroll
+                    for (int r = 0; r < kDenseR; ++r) {
+                        const int o = t0 + lane + 32 * r;
+                        gate[r] = (o >= lo && o <= hi) ? 1.0 : 0.0;
+                    }
+                    const int slot = 2 * (wi * MBHL_NMODE + mi) + seg;
+                    mode_uniform<true>(s_rec + slot * kCoefStride, s_xj[slot], f, lin4, gate, h);
+                }
             }
             if (m_gen) {
-                // general path: lanes 0..5 find, for mode `lane`, the in-band part of the warp tile and the
-                // spline intervals of its two ends
+                // three or more intervals in the chunk (below ~2 mHz): lanes 0..5 find, for mode `lane`, the
+                // in-band part of the warp tile and the spline intervals of its two ends
                 const DenseWalker& w = s_dw[wi];
                 const double* xk = A.knots + ((int64_t)(b0 + wi) * MBHL_NMODE) * A.S;
                 int ja = 0, jb = -1, full = 0;
-                if (kind == 2u) {
+                if (gen) {
                     const DenseMode m = w.mode[lane];
                     const int a = max(kt0, m.k_lo), b = min(kt0 + kWarpTile - 1, m.k_hi);
                     const double* x = xk + lane * A.S;
@@ -280,7 +351,7 @@ __global__ void __launch_bounds__(kDenseThreads, 4) k_dense(DenseArgs A) {
                     const double* x = xk + mi * A.S;
                     const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
                     if (ja_m == jb_m && full_m) {
-                        mode_uniform(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, lin4, h);
+                        mode_uniform<false>(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, lin4, lin4, h);
                     } else {
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
 #pragma unroll

@@ -9,13 +9,22 @@ namespace mbhl {
 constexpr int kCoefStride = MBHL_NQ * 4;   // doubles per (walker, mode, interval) record = 256 B
 constexpr int kSplineHalo = 32;            // overlap rows of the block-parallel tridiagonal solve
 constexpr int kDenseThreads = 128;         // 4 warps per CTA
-constexpr int kDenseR = 4;                 // bins per thread per chunk
+#ifndef MBHL_DENSE_R
+#define MBHL_DENSE_R 4
+#endif
+#ifndef MBHL_DENSE_MINB
+#define MBHL_DENSE_MINB 3
+#endif
+constexpr int kDenseR = MBHL_DENSE_R;      // bins per thread per chunk
 constexpr int kWarpTile = 32 * kDenseR;    // 128 consecutive bins per warp
 constexpr int kChunk = kDenseThreads * kDenseR;   // 512 bins per CTA step
 constexpr int kTileRows = 10;              // rows of a staged data tile: f, w^{A,E,T}, (w Re d, w Im d)^{A,E,T}
 constexpr int kTileDoubles = kTileRows * kChunk;
 constexpr int kTileBytes = kTileDoubles * 8;      // 40 KB, one bulk copy
-constexpr int kMaxW = 8;                   // walkers per CTA tile (upper bound)
+#ifndef MBHL_DENSE_W
+#define MBHL_DENSE_W 8
+#endif
+constexpr int kMaxW = MBHL_DENSE_W;                 // walkers per CTA tile (upper bound)
 constexpr int kPairs = kMaxW * MBHL_NMODE; // (walker, mode) pairs of a CTA tile: one staged coefficient record each
 
 // ---------------------------------------------------------------------------------------------
@@ -337,6 +346,7 @@ struct DenseArgs {
     int G;                   // chunks per CTA
     int n_chunks;
     int n_groups;
+    double inv_df;           // 1 / bin spacing of the init grid
 };
 
 // sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
