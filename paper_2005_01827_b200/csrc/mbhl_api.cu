@@ -151,7 +151,7 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     ctx->launches += 2;
     if (tm) cudaEventRecord(ctx->ev[2], ctx->stream);
     if (with_coef) {
-        k_spline<<<(unsigned)(B * MBHL_NMODE), 128, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
+        k_spline<<<(unsigned)(B * MBHL_NMODE * 2), 128, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
         ctx->launches += 1;
     }
     CU(cudaGetLastError());
@@ -218,10 +218,13 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         return code;
     };
     if (ctx->S < 8 || ctx->S > 8192 || !isfinite(ctx->t0)) return cleanup(MBHL_EINVAL);
-    if (spline_smem_bytes(ctx->S) > 227 * 1024) return cleanup(MBHL_EINVAL);   // S <= ~1550 fits one CTA's shared memory
+    if (spline_smem_bytes(ctx->S) > 227 * 1024) return cleanup(MBHL_EINVAL);   // S <= ~2170 fits one CTA's shared memory
     if (cudaSetDevice(ctx->device) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
+        return cleanup(MBHL_ECUDA);
+    if (cudaFuncSetAttribute(k_spline, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
+        cudaFuncSetAttribute(k_dense, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, kDenseSmemBytes) != cudaSuccess)
         return cleanup(MBHL_ECUDA);

@@ -7,7 +7,6 @@
 namespace mbhl {
 
 constexpr int kCoefStride = MBHL_NQ * 4;   // doubles per (walker, mode, interval) record = 256 B
-constexpr int kSplineHalo = 32;            // overlap rows of the block-parallel tridiagonal solve
 constexpr int kDenseThreads = 128;         // 4 warps per CTA
 #ifndef MBHL_DENSE_R
 #define MBHL_DENSE_R 4
@@ -185,134 +184,180 @@ __global__ void __launch_bounds__(128) k_sparse_eval(const WalkerConst* __restri
 }
 
 // ---------------------------------------------------------------------------------------------
-// a5: not-a-knot cubic spline coefficients.  One CTA of 4 warps per (walker, mode);
-// warp w solves quantities 2w and 2w+1 (the matrix is shared).  Each lane owns a block of consecutive
-// rows of the tridiagonal slope system.  It runs the forward (LU) recurrence from kSplineHalo rows
-// before its block and the backward (UL) recurrence from kSplineHalo rows after it, then combines the
-// two at every owned row (twisted factorisation).  The system is strictly diagonally dominant, so the
-// influence of the cut decays like 0.27^halo for log-spaced knots - below fp64 rounding; blocks that
-// reach row 0 / S-1 use the true not-a-knot rows, so systems with S <= halo are solved exactly.
+// a5: not-a-knot cubic spline coefficients.  The slope system of one
+// (walker, mode) is tridiagonal, strictly diagonally dominant and shared by the 8 splined quantities.  One
+// CTA of 4 warps handles (walker, mode, half) with half = quantities 0-3 or 4-7, so two CTAs fit in one
+// SM's shared memory at S = 1024.  Every recurrence of the Thomas algorithm is contractive here (factors
+// 0.07 for the pivots, 0.27 for both sweeps on log-spaced knots), so each is cut into blocks that start a
+// few rows early from a zero state ("halo"): the influence of the cut is below fp64 rounding after 16
+// (pivots) / 32 (sweeps) rows, and blocks that reach row 0 / S-1 use the true not-a-knot rows.
+//   A. 1/h_r; pivots: thread t owns ceil(S/128) rows: c'_r = u_r / (d_r - a_r c'_{r-1}), 1 division per row
+//   B. b_r = rhs_r / (d_r - a_r c'_{r-1}) for 4 quantities, all rows in parallel
+//   C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows)
+//   D. backward sweep s_r = g_r - c'_r s_{r+1}
+//   E. c_j, d_j of every interval; records written as 128-byte half records
 // coef layout [walker][mode][interval][q][4] = (y_j, s_j, c_j, d_j); phase row: y_j reduced mod 1 cycle.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
 
+constexpr int kSplineQ = 4;              // quantities per CTA
+constexpr int kSplineHaloPivot = 16;
+constexpr int kSplineHaloSweep = 32;
+
 __host__ __device__ inline size_t spline_smem_bytes(int S) {
     const int SP = S + (S >> 5) + 1;
-    return (size_t)(2 + 2 * MBHL_NQ) * SP * sizeof(double);
+    return (size_t)(5 + kSplineQ) * SP * sizeof(double) + (size_t)kSplineQ * S * sizeof(double);
+}
+
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src)
+                 : "memory");
 }
 
 __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ wc, int S, const double* __restrict__ knots,
                                                 const double* __restrict__ y, double* __restrict__ coef) {
     extern __shared__ double sm[];
     const int SP = S + (S >> 5) + 1;
-    double* xk = sm;                     // knots                         [SP]
-    double* cps = sm + SP;               // forward pivots c'_r           [SP]
-    double* rhs = cps + SP;              // right-hand sides              [8][SP]
-    double* wk = rhs + MBHL_NQ * SP;     // forward d'_r, then the slopes [8][SP]
-    const int64_t bm = blockIdx.x;
+    double* xk = sm;                     // knots                                  [SP]
+    double* ih = xk + SP;                // 1 / h_r, h_r = x_{r+1} - x_r          [SP]
+    double* cps = ih + SP;               // pivots c'_r                            [SP]
+    double* ivs = cps + SP;              // 1 / (d_r - a_r c'_{r-1})               [SP]
+    double* mls = ivs + SP;              // a_r / (d_r - a_r c'_{r-1})             [SP]
+    double* A1 = mls + SP;               // b, then g, then the slopes s (in place) [4][SP]
+    double* Y = A1 + kSplineQ * SP;      // y values of the 4 quantities           [4][S], unpadded
+    const int64_t bm = blockIdx.x >> 1;
+    const int half = blockIdx.x & 1;
     const int64_t b = bm / MBHL_NMODE;
     const int mi = (int)(bm - b * MBHL_NMODE);
-    double* cout = coef + bm * (int64_t)(S - 1) * kCoefStride;
+    const int tid = threadIdx.x;
+    double* cout = coef + bm * (int64_t)(S - 1) * kCoefStride + half * (kSplineQ * 4);
     const bool active = wc[b].valid && wc[b].mode[mi].active;
     if (!active) {
-        for (int64_t i = threadIdx.x; i < (int64_t)(S - 1) * kCoefStride; i += blockDim.x) cout[i] = 0.0;
+        for (int idx = tid; idx < (S - 1) * kSplineQ * 2; idx += blockDim.x) {
+            const int j = idx >> 3, i = idx & 7;
+            reinterpret_cast<double2*>(cout + (int64_t)j * kCoefStride)[i] = make_double2(0.0, 0.0);
+        }
         return;
     }
+    // all global reads of this CTA are issued up front as asynchronous copies: knots (group 0), y (group 1)
     const double* xg = knots + bm * S;
-    const double* yg = y + bm * MBHL_NQ * S;
-    for (int i = threadIdx.x; i < S; i += blockDim.x) xk[pad_idx(i)] = xg[i];
+    const double* yg = y + (bm * MBHL_NQ + half * kSplineQ) * S;
+    for (int i = tid; i < S; i += blockDim.x) cp_async8(xk + pad_idx(i), xg + i);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    for (int i = tid; i < kSplineQ * S; i += blockDim.x) cp_async8(Y + i, yg + i);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
     __syncthreads();
-    // right-hand sides of the slope system, all rows in parallel
-    for (int idx = threadIdx.x; idx < MBHL_NQ * S; idx += blockDim.x) {
+    // matrix row r: (lower a, diag d, upper u)
+    auto mat = [&](int r, double& a, double& d, double& u) {
+        if (r == 0) {
+            const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
+            a = 0.0; d = h1; u = h0 + h1;
+        } else if (r == S - 1) {
+            const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
+            a = hm + hn; d = hn; u = 0.0;
+        } else {
+            const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
+            a = hr; d = 2.0 * (hl + hr); u = hl;
+        }
+    };
+    // A. reciprocal spacings and pivots
+    for (int r = tid; r < S - 1; r += blockDim.x) ih[pad_idx(r)] = 1.0 / (xk[pad_idx(r + 1)] - xk[pad_idx(r)]);
+    {
+        const int m = (S + (int)blockDim.x - 1) / (int)blockDim.x;
+        const int own0 = tid * m, own1 = min(S, own0 + m);
+        if (own0 < own1) {
+            double cp = 0.0;
+            for (int r = max(0, own0 - kSplineHaloPivot); r < own1; ++r) {
+                double a, d, u;
+                mat(r, a, d, u);
+                const double inv = 1.0 / (d - a * cp);
+                cp = u * inv;
+                if (r >= own0) { cps[pad_idx(r)] = cp; ivs[pad_idx(r)] = inv; mls[pad_idx(r)] = a * inv; }
+            }
+        }
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    // B. scaled right-hand sides of the slope system, all rows in parallel
+    for (int idx = tid; idx < kSplineQ * S; idx += blockDim.x) {
         const int q = idx / S, r = idx - q * S;
-        const double* yq = yg + q * S;
+        const double* yq = Y + q * S;
         double v;
         if (r == 0) {
             const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
-            const double d0 = (yq[1] - yq[0]) / h0, d1 = (yq[2] - yq[1]) / h1;
+            const double d0 = (yq[1] - yq[0]) * ih[pad_idx(0)], d1 = (yq[2] - yq[1]) * ih[pad_idx(1)];
             v = ((3.0 * h0 + 2.0 * h1) * h1 * d0 + h0 * h0 * d1) / (h0 + h1);
         } else if (r == S - 1) {
             const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
-            const double dm = (yq[S - 1] - yq[S - 2]) / hm, dn = (yq[S - 2] - yq[S - 3]) / hn;
+            const double dm = (yq[S - 1] - yq[S - 2]) * ih[pad_idx(S - 2)], dn = (yq[S - 2] - yq[S - 3]) * ih[pad_idx(S - 3)];
             v = (hm * hm * dn + (2.0 * hn + 3.0 * hm) * hn * dm) / (hn + hm);
         } else {
             const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
-            v = 3.0 * (hr * ((yq[r] - yq[r - 1]) / hl) + hl * ((yq[r + 1] - yq[r]) / hr));
+            const double yr = yq[r];
+            v = 3.0 * (hr * ((yr - yq[r - 1]) * ih[pad_idx(r - 1)]) + hl * ((yq[r + 1] - yr) * ih[pad_idx(r)]));
         }
-        rhs[q * SP + pad_idx(r)] = v;
+        A1[q * SP + pad_idx(r)] = v * ivs[pad_idx(r)];
     }
     __syncthreads();
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int qa = 2 * warp, qb = 2 * warp + 1;
-    const int m = (S + 31) / 32;                       // rows per lane
-    const int own0 = lane * m, own1 = min(S, own0 + m);
-    if (own0 < own1) {
-        const int r0 = max(0, own0 - kSplineHalo), r1 = min(S, own1 + kSplineHalo);
-        // matrix row r: (lower a, diag d, upper u)
-        auto mat = [&](int r, double& a, double& d, double& u) {
-            if (r == 0) {
-                const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
-                a = 0.0; d = h1; u = h0 + h1;
-            } else if (r == S - 1) {
-                const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
-                a = hm + hn; d = hn; u = 0.0;
-            } else {
-                const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
-                a = hr; d = 2.0 * (hl + hr); u = hl;
+    // C, D. sweeps in place: warp = quantity, lane = block of rows.  A lane first copies the halo rows it needs
+    // from its neighbour's block into registers, so the neighbour may overwrite them afterwards.
+    {
+        const int q = tid >> 5, lane = tid & 31;
+        const int m = (S + 31) / 32;
+        const int own0 = lane * m, own1 = min(S, own0 + m);
+        double* aq = A1 + q * SP;
+        double halo[kSplineHaloSweep];
+#pragma unroll
+        for (int i = 0; i < kSplineHaloSweep; ++i) {
+            const int r = own0 - kSplineHaloSweep + i;
+            halo[i] = (r >= 0 && r < S) ? aq[pad_idx(r)] : 0.0;
+        }
+        __syncwarp();
+        if (own0 < own1) {
+            double g = 0.0;
+#pragma unroll
+            for (int i = 0; i < kSplineHaloSweep; ++i) {
+                const int r = own0 - kSplineHaloSweep + i;
+                if (r >= 0) g = fma(-mls[pad_idx(r)], g, halo[i]);
             }
-        };
-        // forward recurrence: s_r + cp_r s_{r+1} = dp_r
-        double cp = 0.0, gA = 0.0, gB = 0.0;           // values at row r-1
-        double cp_e = 0.0, gA_e = 0.0, gB_e = 0.0;     // values at row own0-1 (kept in registers)
-        for (int r = r0; r < own1 - 1; ++r) {
-            double a, d, u;
-            mat(r, a, d, u);
-            const double inv = 1.0 / (d - a * cp);
-            cp = u * inv;
-            gA = (rhs[qa * SP + pad_idx(r)] - a * gA) * inv;
-            gB = (rhs[qb * SP + pad_idx(r)] - a * gB) * inv;
-            if (r == own0 - 1) { cp_e = cp; gA_e = gA; gB_e = gB; }
-            if (r >= own0) {
-                cps[pad_idx(r)] = cp;                   // all four warps write identical values
-                wk[qa * SP + pad_idx(r)] = gA;
-                wk[qb * SP + pad_idx(r)] = gB;
+            for (int r = own0; r < own1; ++r) {
+                g = fma(-mls[pad_idx(r)], g, aq[pad_idx(r)]);
+                aq[pad_idx(r)] = g;
             }
         }
-        // backward recurrence: s_r + bp_r s_{r-1} = ep_r, combined with the forward one at owned rows
-        double bp = 0.0, eA = 0.0, eB = 0.0;           // values at row r+1
-        for (int r = r1 - 1; r >= own0; --r) {
-            double a, d, u;
-            mat(r, a, d, u);
-            const double rA = rhs[qa * SP + pad_idx(r)], rB = rhs[qb * SP + pad_idx(r)];
-            if (r < own1) {
-                double fc, fA, fB;                      // forward quantities of row r-1
-                if (r == own0) { fc = cp_e; fA = gA_e; fB = gB_e; }
-                else { fc = cps[pad_idx(r - 1)]; fA = wk[qa * SP + pad_idx(r - 1)]; fB = wk[qb * SP + pad_idx(r - 1)]; }
-                const double invD = 1.0 / (d - a * fc - u * bp);
-                const double sA = (rA - a * fA - u * eA) * invD;
-                const double sB = (rB - a * fB - u * eB) * invD;
-                wk[qa * SP + pad_idx(r)] = sA;          // d'_r of this row is no longer needed
-                wk[qb * SP + pad_idx(r)] = sB;
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < kSplineHaloSweep; ++i) {
+            const int r = own1 + i;
+            halo[i] = (r < S) ? aq[pad_idx(r)] : 0.0;
+        }
+        __syncwarp();
+        if (own0 < own1) {
+            double sl = 0.0;
+#pragma unroll
+            for (int i = kSplineHaloSweep - 1; i >= 0; --i) {
+                const int r = own1 + i;
+                if (r < S) sl = fma(-cps[pad_idx(r)], sl, halo[i]);
             }
-            const double inv = 1.0 / (d - u * bp);
-            bp = a * inv;
-            eA = (rA - u * eA) * inv;
-            eB = (rB - u * eB) * inv;
+            for (int r = own1 - 1; r >= own0; --r) {
+                sl = fma(-cps[pad_idx(r)], sl, aq[pad_idx(r)]);
+                aq[pad_idx(r)] = sl;
+            }
         }
     }
     __syncthreads();
-    // coefficients: one (interval, quantity) per thread, 32 B each, consecutive threads -> consecutive records
-    for (int idx = threadIdx.x; idx < (S - 1) * MBHL_NQ; idx += blockDim.x) {
-        const int j = idx / MBHL_NQ, q = idx - j * MBHL_NQ;
-        const double h = xk[pad_idx(j + 1)] - xk[pad_idx(j)];
-        double y0 = yg[q * S + j];
-        const double y1 = yg[q * S + j + 1];
-        const double s0 = wk[q * SP + pad_idx(j)], s1 = wk[q * SP + pad_idx(j + 1)];
-        const double dl = (y1 - y0) / h;
-        const double cc = (3.0 * dl - 2.0 * s0 - s1) / h;
-        const double dd = (s0 + s1 - 2.0 * dl) / (h * h);
-        if (q == 1) y0 -= rint(y0);
+    // E. coefficients: one (interval, quantity) per thread, 32 B each; 4 consecutive threads write a 128-byte half record
+    for (int idx = tid; idx < (S - 1) * kSplineQ; idx += blockDim.x) {
+        const int j = idx >> 2, q = idx & 3;
+        const double hinv = ih[pad_idx(j)];
+        double y0 = Y[q * S + j];
+        const double y1 = Y[q * S + j + 1];
+        const double s0 = A1[q * SP + pad_idx(j)], s1 = A1[q * SP + pad_idx(j + 1)];
+        const double dl = (y1 - y0) * hinv;
+        const double cc = (3.0 * dl - 2.0 * s0 - s1) * hinv;
+        const double dd = (s0 + s1 - 2.0 * dl) * (hinv * hinv);
+        if (half == 0 && q == 1) y0 -= rint(y0);
         double2* o = reinterpret_cast<double2*>(cout + (int64_t)j * kCoefStride + q * 4);
         o[0] = make_double2(y0, s0);
         o[1] = make_double2(cc, dd);
