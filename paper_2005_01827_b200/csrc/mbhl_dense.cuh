@@ -366,19 +366,33 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                     }
                 }
             }
-            // inner products of this walker over the warp's 128 bins
+            // inner products of this walker over the warp's 128 bins (one accumulator pair per bin: independent chains)
+            double dhr[kDenseR], hhr[kDenseR];
+#pragma unroll
+            for (int r = 0; r < kDenseR; ++r) { dhr[r] = 0.0; hhr[r] = 0.0; }
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                double ww[kDenseR], wre[kDenseR], wim[kDenseR], n2[kDenseR];
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) {
+                    ww[r] = sf[(1 + ch) * kChunk + lane + 32 * r];
+                    wre[r] = sf[(4 + 2 * ch) * kChunk + lane + 32 * r];
+                    wim[r] = sf[(5 + 2 * ch) * kChunk + lane + 32 * r];
+                }
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) n2[r] = h[r][2 * ch] * h[r][2 * ch];
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) dhr[r] = fma(wre[r], h[r][2 * ch], dhr[r]);
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) n2[r] = fma(h[r][2 * ch + 1], h[r][2 * ch + 1], n2[r]);
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) dhr[r] = fma(wim[r], h[r][2 * ch + 1], dhr[r]);
+#pragma unroll
+                for (int r = 0; r < kDenseR; ++r) hhr[r] = fma(ww[r], n2[r], hhr[r]);
+            }
             double dh = 0.0, hh = 0.0;
 #pragma unroll
-            for (int r = 0; r < kDenseR; ++r) {
-#pragma unroll
-                for (int ch = 0; ch < 3; ++ch) {
-                    const double ww = sf[(1 + ch) * kChunk + lane + 32 * r];
-                    const double wre = sf[(4 + 2 * ch) * kChunk + lane + 32 * r];
-                    const double wim = sf[(5 + 2 * ch) * kChunk + lane + 32 * r];
-                    dh = fma(wre, h[r][2 * ch], fma(wim, h[r][2 * ch + 1], dh));
-                    hh = fma(ww, fma(h[r][2 * ch], h[r][2 * ch], h[r][2 * ch + 1] * h[r][2 * ch + 1]), hh);
-                }
-            }
+            for (int r = 0; r < kDenseR; ++r) { dh += dhr[r]; hh += hhr[r]; }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 dh += __shfl_down_sync(0xffffffffu, dh, o);

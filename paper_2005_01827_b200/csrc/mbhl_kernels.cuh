@@ -396,11 +396,24 @@ struct DenseArgs {
 
 // sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
 // (Chebyshev-node interpolation in 50-digit arithmetic; max error 2.6e-17 / 1.0e-16 before rounding).
-constexpr double kS0 = 1.5707963267948966, kS1 = -0.6459640975062443, kS2 = 0.07969262624604301,
-                 kS3 = -0.004681754132340976, kS4 = 0.0001604411507421909, kS5 = -3.59864335298231e-06,
-                 kS6 = 5.633933781537854e-08;
-constexpr double kC1 = -1.2337005501361513, kC2 = 0.25366950789986475, kC3 = -0.02086348073494657,
-                 kC4 = 0.000919259950041661, kC5 = -2.520013526428479e-05, kC6 = 4.6552961874867623e-07;
+// Kept in the constant bank so that DFMA reads them as c[][] operands (as immediates each costs two moves per use).
+__constant__ double c_sc[13] = {1.5707963267948966, -0.6459640975062443, 0.07969262624604301, -0.004681754132340976,
+                                0.0001604411507421909, -3.59864335298231e-06, 5.633933781537854e-08,
+                                -1.2337005501361513, 0.25366950789986475, -0.02086348073494657,
+                                0.000919259950041661, -2.520013526428479e-05, 4.6552961874867623e-07};
+#define kS0 c_sc[0]
+#define kS1 c_sc[1]
+#define kS2 c_sc[2]
+#define kS3 c_sc[3]
+#define kS4 c_sc[4]
+#define kS5 c_sc[5]
+#define kS6 c_sc[6]
+#define kC1 c_sc[7]
+#define kC2 c_sc[8]
+#define kC3 c_sc[9]
+#define kC4 c_sc[10]
+#define kC5 c_sc[11]
+#define kC6 c_sc[12]
 constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
 
 // sin and cos of p4 quarter turns (angle = p4 pi/2), any |p4| < 2^51.  No conversions, no divides: the

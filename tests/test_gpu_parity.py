@@ -265,3 +265,34 @@ def test_loglike_parity_config1_sampled_walkers(table):
     ref = L.loglike_parts(table, wl["injections"][0], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])[2]
     assert abs(inj - ref) <= 1e-6 * (1.0 + abs(ref))
     M.mbhl_free(ctx)
+
+
+def test_loglike_parity_config2_full_size_in_the_bench_launch_configuration(table):
+    # BASELINE config 2 at full size (B = 1024, S = 1024, N = 4 197 160), the batch and launch shape bench.py times:
+    # one walker per injection group plus the group boundaries are checked by the oracle one by one, the rest
+    # through properties that hold at any size.
+    tf = lambda p, f, S: L.template(table, p, f, S)
+    wl = W.build(2, tf)
+    B = wl["params"].shape[0]
+    assert B == 1024 and wl["freqs"].size == 4197160 and wl["S"] == 1024
+    ctx = make_ctx(wl, max_batch=B)
+    p = dev(wl["params"])
+    dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, p)]
+    dd = M.mbhl_data_norm(ctx)
+    assert np.all(np.isfinite(ll)) and np.all(hh > 0.0)
+    assert np.max(np.abs(ll - (dh - 0.5 * hh - 0.5 * dd)) / (dd + hh)) <= 1e-12       # eq. 2
+    assert np.array_equal(M.mbhl_loglike(ctx, p).cpu().numpy(), ll)                     # bitwise reproducible
+    # a walker's result does not depend on its position in the batch or on its tile mates (tiles of 8 walkers)
+    perm = np.random.default_rng(7).permutation(B)
+    assert np.array_equal(M.mbhl_loglike(ctx, dev(wl["params"][perm])).cpu().numpy(), ll[perm])
+    sub = [3, 341, 342, 700, 1023]
+    # a small batch takes another launch shape (chunks per CTA), i.e. another summation order
+    ll_sub = M.mbhl_loglike(ctx, dev(wl["params"][sub])).cpu().numpy()
+    assert np.max(np.abs(ll_sub - ll[sub]) / (dd + hh[sub])) <= 1e-13
+    pairs, bins = M.mbhl_last_work(ctx)
+    assert 0 < bins <= len(sub) * wl["freqs"].size and bins <= pairs <= 6 * bins
+    for b in (0, 341, 342, 683, 1023):
+        rdh, rhh, rll = L.loglike_parts(table, wl["params"][b], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])
+        assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (b, ll[b], rll)
+        assert abs(hh[b] - rhh) <= 1e-8 * rhh, (b, hh[b], rhh)
+    M.mbhl_free(ctx)
