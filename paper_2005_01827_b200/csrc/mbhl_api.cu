@@ -51,13 +51,18 @@ struct DensePlan {
     int W, G, n_tiles, n_groups;
 };
 
+#ifndef MBHL_DENSE_MAXG
+#define MBHL_DENSE_MAXG 32
+#endif
+constexpr int kDenseMaxG = MBHL_DENSE_MAXG;   // chunks per CTA at most: amortises a CTA's start-up over ~0.5 ms of work
+
 DensePlan dense_plan(int64_t B, int n_chunks) {
     DensePlan p;
     int64_t w = B * (int64_t)n_chunks / 4096;
     p.W = (int)(w < 1 ? 1 : (w > kMaxW ? kMaxW : w));
     p.n_tiles = (int)((B + p.W - 1) / p.W);
     int64_t g = (int64_t)p.n_tiles * n_chunks / 8192;
-    p.G = (int)(g < 1 ? 1 : (g > 16 ? 16 : g));
+    p.G = (int)(g < 1 ? 1 : (g > kDenseMaxG ? kDenseMaxG : g));
     p.n_groups = (n_chunks + p.G - 1) / p.G;
     return p;
 }

@@ -393,12 +393,12 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
             double dh = 0.0, hh = 0.0;
 #pragma unroll
             for (int r = 0; r < kDenseR; ++r) { dh += dhr[r]; hh += hhr[r]; }
+            // lanes 0-15 collect <d|h>, lanes 16-31 collect <h|h>: one exchange, then a 4-step tree per half
+            const bool upper = lane >= 16;
+            double v = (upper ? hh : dh) + __shfl_xor_sync(0xffffffffu, upper ? dh : hh, 16);
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                dh += __shfl_down_sync(0xffffffffu, dh, o);
-                hh += __shfl_down_sync(0xffffffffu, hh, o);
-            }
-            if (lane == 0) { s_acc[warp][wi][0] += dh; s_acc[warp][wi][1] += hh; }
+            for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if ((lane & 15) == 0) s_acc[warp][wi][lane >> 4] += v;
         }
     }
     __syncthreads();
