@@ -112,6 +112,149 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def _device_setup():
+    import torch
+    from paper_2005_01827_b200 import binding as M
+    from paper_2005_01827_b200 import build as mbuild
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    mbuild.build()
+    M.lib()
+    return torch, M, torch.device("cuda", local), local
+
+
+def _fp64_probe(torch, M, dev):
+    sink = torch.zeros(8, dtype=torch.float64, device=dev)
+    blocks, threads, iters = 148 * 8, 256, 20000
+    M.mbhl_dfma_probe(blocks, threads, 200, sink)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    M.mbhl_dfma_probe(blocks, threads, iters, sink)
+    p1.record()
+    torch.cuda.synchronize()
+    return 2.0 * blocks * threads * iters * 8 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+
+def _hbm_peak():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
+
+
+def run_sparse_isolation(args):
+    """BASELINE.json configs[3]: B = 16384 parameter sets, steps a1-a5 only (mbhl_sparse), no dense stage."""
+    torch, M, dev, local = _device_setup()
+    from paper_2005_01827_b200 import workloads as W
+    S, B = 1024, args.batch or 16384
+    freqs = W.grid(1.33, int(0.1 * 1.33 * W.YEAR_JULIAN_S), 0.0)
+    N = freqs.size
+    ctx = M.mbhl_init(torch.as_tensor(freqs, device=dev), torch.zeros((3, N, 2), dtype=torch.float64, device=dev),
+                      torch.ones((3, N), dtype=torch.float64, device=dev), sparse_points=S, max_batch=B, device=local)
+    params = torch.as_tensor(W.sparse_batch(B), device=dev)
+    M.mbhl_enable_stage_timing(ctx, True)
+    for _ in range(max(args.warmup, 3)):
+        M.mbhl_sparse(ctx, params, outputs=False)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    M.mbhl_stage_times(ctx)
+    launches0 = M.mbhl_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        M.mbhl_sparse(ctx, params, outputs=False)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    stage = M.mbhl_stage_times(ctx)
+    launches = M.mbhl_launch_count(ctx) - launches0
+    clocks = sampler.stop()
+    # algorithmic HBM bytes per parameter set (DESIGN.md section 7): knots + y written once and read once by the
+    # spline kernel, coefficient records written once
+    bytes_set = 6 * S * (8 + 64) * 2 + 6 * (S - 1) * 256
+    hbm, hbm_src = _hbm_peak()
+    spline_bytes = B * (6 * S * (8 + 64) + 6 * (S - 1) * 256)       # what k_spline itself reads and writes
+    achieved = spline_bytes / (stage[2] * 1e-3) / 1e9
+    fp64_peak = _fp64_probe(torch, M, dev)
+    flops_set = 1730.0 * 6 * S                                       # SURVEY.md 8(d): ~1600 + 130 FLOPs per knot
+    print(json.dumps({
+        "metric": "parameter sets/sec (sparse stage only)", "value": B / (ms * 1e-3), "unit": "sets/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[3]: B={B} parameter sets (config-0 priors, M_T log-uniform 1e5-1e8), 6 modes x S={S} knots; "
+                               "per-walker constants + PhenomHM + response + spline coefficients, no dense stage",
+                   "l2": "outputs larger than L2 (coefficient records %.1f GB per step)" % (B * 6 * (S - 1) * 256 / 1e9),
+                   "stage_ms": {k: float(v) for k, v in zip(("consts", "sparse", "spline"), stage[:3])}},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "k_spline", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
+                     "traffic": None, "peak_source": hbm_src, "algorithmic_bytes_per_launch": spline_bytes,
+                     "whole_stage": {"hbm_bound_ms": B * bytes_set / (hbm * 1e9) * 1e3, "fp64_bound_ms": B * flops_set / (fp64_peak * 1e12) * 1e3,
+                                     "measured_ms": ms, "fp64_peak_tflops": fp64_peak}}}))
+    M.mbhl_free(ctx)
+
+
+def run_dense_sweep(args):
+    """BASELINE.json configs[4]: dense grid N x batch B sweep, random priors with M_T log-uniform [1e5, 1e8]; one line per point."""
+    torch, M, dev, local = _device_setup()
+    from paper_2005_01827_b200 import workloads as W
+    S = 1024
+    fp64_peak = _fp64_probe(torch, M, dev)
+    hbm, _ = _hbm_peak()
+    all_params = W.sparse_batch(4096, seed_offset=4)
+    rng = np.random.default_rng(W.SEED0 + 4)
+    for logn in (16, 18, 20, 22, 23):
+        N = 1 << logn
+        df = 0.1 / N
+        freqs = (1.0 + np.arange(N, dtype=np.float64)) * df           # N bins ending at 0.1 Hz
+        psd = W.scird_psd_aet(freqs)
+        f_d, psd_d = torch.as_tensor(freqs, device=dev), torch.as_tensor(psd, device=dev)
+        ctx0 = M.mbhl_init(f_d, torch.zeros((3, N, 2), dtype=torch.float64, device=dev), torch.ones((3, N), dtype=torch.float64, device=dev),
+                           sparse_points=S, device=local)
+        scale_t = (1.0 / df) / (1.33 * W.YEAR_JULIAN_S)             # t_ref was drawn as a fraction of 1.33 yr: same fraction of T_obs = 1/df
+        inj = all_params[:1].copy()
+        inj[0, 10] *= scale_t
+        data = M.mbhl_template(ctx0, torch.as_tensor(inj, device=dev))[0].cpu().numpy() + W.noise(rng, psd, df)
+        M.mbhl_free(ctx0)
+        ctx = M.mbhl_init(f_d, torch.as_tensor(data, device=dev), psd_d, sparse_points=S, max_batch=4096, device=local)
+        M.mbhl_enable_stage_timing(ctx, True)
+        for B in (1, 16, 256, 1024, 4096):
+            p = all_params[:B].copy()
+            p[:, 10] *= scale_t
+            params = torch.as_tensor(p, device=dev)
+            logL = torch.empty(B, dtype=torch.float64, device=dev)
+            for _ in range(3):
+                M.mbhl_loglike(ctx, params, logL)
+            torch.cuda.synchronize()
+            M.mbhl_stage_times(ctx)
+            steps = args.steps
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                M.mbhl_loglike(ctx, params, logL)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            stage = M.mbhl_stage_times(ctx)
+            pairs, bins = M.mbhl_last_work(ctx)
+            flops = FLOP_PER_PAIR * pairs + FLOP_PER_BIN * bins
+            fp64_ms = flops / (fp64_peak * 1e12) * 1e3
+            hbm_ms = (80.0 * N * max(1, (B + 7) // 8) + B * 6 * (S - 1) * 256) / (hbm * 1e9) * 1e3
+            print(json.dumps({"metric": METRIC, "value": B / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1, "steps": steps, "ms_per_step": ms,
+                              "dtype": "f64", "data": "synthetic",
+                              "config": {"workload": f"BASELINE.json configs[4] point: N=2^{logn} bins ending at 0.1 Hz, B={B}, S={S}",
+                                         "active_pairs_per_step": pairs, "active_bins_per_step": bins,
+                                         "stage_ms": {k: float(v) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
+                              "roofline": {"bound": "alu" if fp64_ms >= hbm_ms else "hbm", "dense_fp64_bound_ms": fp64_ms, "dense_hbm_bound_ms": hbm_ms,
+                                           "frac": max(fp64_ms, hbm_ms) / stage[3], "frac_of_step": max(fp64_ms, hbm_ms) / ms,
+                                           "fp64_peak_tflops": fp64_peak},
+                              "finite": bool(torch.isfinite(logL).all().item())}), flush=True)
+        M.mbhl_free(ctx)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -265,12 +408,21 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=(0, 1, 2))
+    ap.add_argument("--config", type=int, default=2, choices=(0, 1, 2, 3, 4),
+                    help="BASELINE.json config; 0-2 are likelihood workloads (2 = default bench line), 3 = sparse-stage isolation, "
+                         "4 = dense N x B sweep (one JSON line per point)")
+    ap.add_argument("--batch", type=int, default=0, help="config 3 only: number of parameter sets (default 16384)")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     if args.impl == "reference":
+        if args.config > 2:
+            raise SystemExit("--impl reference times the likelihood configs 0-2")
         run_reference(args)
+    elif args.config == 3:
+        run_sparse_isolation(args)
+    elif args.config == 4:
+        run_dense_sweep(args)
     else:
         if int(os.environ.get("WORLD_SIZE", "1")) > 1 or args.gpus > 1:
             args.cpu_baseline = args.cpu_baseline and int(os.environ.get("RANK", "0")) == 0 and int(os.environ.get("WORLD_SIZE", "1")) == 1

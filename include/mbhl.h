@@ -125,7 +125,8 @@ int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins);
  * around its five stages; mbhl_stage_times synchronises the stream, returns the MEAN milliseconds per stage
  * over the calls made since the previous mbhl_stage_times / enable (at most the last 64) and resets the
  * count: ms[0] per-walker constants, ms[1] sparse evaluation, ms[2] spline solve, ms[3] fused dense kernel,
- * ms[4] final reduction.  Returns MBHL_EINVAL if timing is off or no call was made.                       */
+ * ms[4] final reduction (mbhl_sparse is timed too, with ms[3] = ms[4] = 0).  Returns MBHL_EINVAL if timing
+ * is off or no call was made.                                                                            */
 int mbhl_enable_stage_timing(mbhl_ctx* ctx, int32_t on);
 int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]);
 

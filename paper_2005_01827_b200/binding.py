@@ -136,8 +136,12 @@ def mbhl_template(ctx, params, freqs_out=None, direct=False):
     return torch.view_as_complex(out)
 
 
-def mbhl_sparse(ctx, params, want_coef=True):
+def mbhl_sparse(ctx, params, want_coef=True, outputs=True):
+    """Steps a1-a5 only.  outputs=False passes NULL for all three outputs (results stay in the workspace)."""
     B = int(params.shape[0])
+    if not outputs:
+        _check(lib().mbhl_sparse(ctx, _ptr(params), B, None, None, None), ctx)
+        return None
     S = int(lib().mbhl_sparse_points(ctx))
     dev = params.device
     knots = torch.empty((B, NMODE, S), dtype=torch.float64, device=dev)

@@ -435,6 +435,10 @@ int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, d
     const WsLayout L = layout(ctx, B);
     rc = run_sparse(ctx, params, B, base, L, true);
     if (rc != MBHL_OK) return rc;
+    if (ctx->timing) {   // stages 3 and 4 (dense, reduce) do not run here: zero-length intervals
+        for (int i = 3; i < 6; ++i) cudaEventRecord(ctx->ev[i], ctx->stream);
+        ctx->n_timed += 1;
+    }
     const size_t nk = (size_t)B * MBHL_NMODE * ctx->S;
     if (knots) CU(cudaMemcpyAsync(knots, base + L.knots, nk * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     if (y) {

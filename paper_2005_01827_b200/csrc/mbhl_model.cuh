@@ -344,6 +344,33 @@ __device__ inline void solve5(double A[5][5], double b[5]) {
     }
 }
 
+// Root of a continuous function on a bracket [a, b] with fn(a) = fa and fn(b) = fb of opposite signs
+// (Illinois variant of regula falsi, bisection when the secant leaves the bracket).  Stops when the bracket
+// is a few ulps wide or |fn| <= ftol; returns the end point whose sign matches fb.
+template <typename F>
+__device__ inline double bracketed_root(F fn, double a, double fa, double b, double fb, double ftol) {
+    if (fb == 0.0) return b;
+    const bool up = fb > 0.0;                            // sign of the kept end point
+    int side = 0;
+    for (int it = 0; it < 200; ++it) {
+        if (fabs(b - a) <= 4.5e-16 * fmax(fabs(a), fabs(b))) break;
+        double x = (a * fb - b * fa) / (fb - fa);
+        if (!((x > a && x < b) || (x < a && x > b))) x = 0.5 * (a + b);
+        const double fx = fn(x);
+        if ((fx > 0.0) == up || fx == 0.0) {
+            b = x; fb = fx;
+            if (fabs(fx) <= ftol) break;
+            if (side == 1) fa *= 0.5;
+            side = 1;
+        } else {
+            a = x; fa = fx;
+            if (side == -1) fb *= 0.5;
+            side = -1;
+        }
+    }
+    return b;
+}
+
 __device__ inline void build_walker(const double* __restrict__ p, double t0, double f_min, double f_max, int S,
                                     uint32_t mode_mask, WalkerConst& c) {
     const double M_T = p[0], q_in = p[1], a1 = p[2], a2 = p[3], D_L = p[4];
@@ -491,12 +518,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
         };
         double lo = c.f_peak, hi = c.fRD + 4.0 * w;
         for (int it = 0; it < 64 && g(hi) > 0.0; ++it) hi += w;
-        for (int it = 0; it < 200; ++it) {
-            const double mid = 0.5 * (lo + hi);
-            if (mid == lo || mid == hi) break;
-            if (g(mid) > 0.0) lo = mid; else hi = mid;
-        }
-        c.f_ref = 0.5 * (lo + hi);
+        c.f_ref = bracketed_root(g, lo, g(lo), hi, g(hi), 0.0);      // g > 0 at lo, g <= 0 at hi
     }
     // phase connections and alignment
     c.f_mr = 0.5 * c.fRD;
@@ -595,7 +617,15 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
         mc.active = 0;
         mc.f_lo = mc.f_hi = mc.dlog = mc.inv_dlog = mc.ln_flo = 0.0;
     }
-    // bands (O5)
+    // bands (O5).  On the inspiral branch of the phase map t_lm(f) = t_22(2 f / m), so the
+    // six roots of t_lm(f) = 0 are images of ONE root x0 of t_22 in (2,2) geometric frequency, found once.
+    auto t22 = [&](double x22) {
+        double p_, d_;
+        psi22(c, x22, &p_, &d_);
+        return c.t_coal + c.M_s * d_ * (1.0 / kTwoPi);
+    };
+    const double t_top = t22(kFPhiIns);                 // t_lm at the end of every mode's inspiral branch
+    double x0 = -1.0;
     for (int mi = 0; mi < MBHL_NMODE; ++mi) {
         if (!((mode_mask >> mi) & 1u)) continue;
         ModeConst& mc = c.mode[mi];
@@ -603,18 +633,17 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
         const double f_top = 0.5 * m * kFPhiIns / c.M_s;
         const double f_hi = fmin(f_max, 0.2 * fmax(1.0, 0.5 * m) / c.M_s);
         double f_lo;
-        if (t_of_f(c, mi, f_min) >= 0.0) {
+        const double t_min = t_of_f(c, mi, f_min);
+        if (t_min >= 0.0) {
             f_lo = f_min;
-        } else if (f_top <= f_min || t_of_f(c, mi, f_top) < 0.0) {
+        } else if (f_top <= f_min || t_top < 0.0) {
             f_lo = fmax(f_top, f_min);
         } else {
-            double lo = f_min, hi = f_top;
-            for (int it = 0; it < 200; ++it) {
-                const double mid = 0.5 * (lo + hi);
-                if (mid <= lo || mid >= hi) break;
-                if (t_of_f(c, mi, mid) < 0.0) lo = mid; else hi = mid;
+            if (x0 < 0.0) {
+                const double xa = mc.aP[0] * (f_min * c.M_s);        // t22(xa) = t_min < 0 <= t_top
+                x0 = bracketed_root(t22, xa, t_min, kFPhiIns, t_top, 4e-16 * fabs(c.t_coal) + 1e-12);
             }
-            f_lo = hi;
+            f_lo = fmax(f_min, x0 * (0.5 * m) / c.M_s);
         }
         if (f_hi > f_lo) {
             mc.active = 1;
