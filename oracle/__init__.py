@@ -17,6 +17,8 @@ Pins (tests/test_oracle_*.py, -m "not gpu"):
                 P11 rigid triangle, P12 T-channel suppression
   chain         P14 spline-vs-direct template, P15 exact linear phase term,
                 P18 independent mpmath re-evaluation of a tiny case
+  sampler side  (oracle/sampler.py) Table I box, Philox known answers, stretch-move
+                z density, detailed balance of move + swap on a tempered Gaussian, <d|h> linear over modes
 Parity unpinned: fidelity of the model *numbers* to the published PhenomD /
 PhenomHM calibration (the tables are not available offline).
 """

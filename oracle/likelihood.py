@@ -183,3 +183,17 @@ def loglike_direct_residual(table, params, freqs, data, psd, S, t0=0.0, mode="sp
     h = template(table, params, freqs, S, t0, mode)
     r = data - h
     return -0.5 * inner(r, r, w)
+
+
+def mode_products(table, params, freqs, data, psd, S, t0=0.0):
+    """Per-mode inner products (Table III :292-300): for each mode evaluated in isolation,
+    (<d|h_lm>, <h_lm|h_lm>); the optimal SNR of the mode alone is <h_lm|h_lm>^(1/2).
+    Returns two arrays of length 6 in the mode order of PAPER.md:122."""
+    w = weights(freqs, psd)
+    dh = np.zeros(len(MODES))
+    hh = np.zeros(len(MODES))
+    for i in range(len(MODES)):
+        h = template(table, params, freqs, S, t0, mode_mask=1 << i)
+        dh[i] = inner(data, h, w)
+        hh[i] = inner(h, h, w)
+    return dh, hh

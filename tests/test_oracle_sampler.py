@@ -1,0 +1,112 @@
+"""Pins of oracle/sampler.py and of the per-mode products: Table I, Philox known answers, the
+stretch proposal's distribution, detailed balance on a Gaussian target, linearity of <d|h> over the modes."""
+import math
+import os
+
+import numpy as np
+
+from oracle import likelihood as L
+from oracle import sampler as S
+from paper_2005_01827_b200 import workloads as W
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def golden():
+    out = {}
+    for line in open(os.path.join(HERE, "golden", "paper_tables.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+def test_prior_box_is_table_one():
+    g = golden()
+    lo, hi = S.PRIOR_LO, S.PRIOR_HI
+    assert abs(math.exp(lo[0]) / g["prior_MT_lo"] - 1) < 1e-14
+    assert abs(math.exp(hi[0]) / g["prior_MT_hi"] - 1) < 1e-14
+    assert (lo[1], hi[1]) == (g["prior_q_lo"], g["prior_q_hi"])
+    assert (lo[2], hi[2], lo[3], hi[3]) == (g["prior_a_lo"], g["prior_a_hi"], g["prior_a_lo"], g["prior_a_hi"])
+    assert abs(math.exp(lo[4]) / g["DL_z0.01"] - 1) < 1e-14 and abs(math.exp(hi[4]) / g["DL_z100"] - 1) < 1e-14
+    assert (lo[5], lo[7], lo[9]) == (0.0, 0.0, 0.0) and hi[5] == hi[7] == 2 * math.pi and hi[9] == math.pi
+    assert (lo[6], hi[6], lo[8], hi[8]) == (-1.0, 1.0, -1.0, 1.0)
+    assert abs(math.exp(lo[10]) / g["prior_tref_lo"] - 1) < 1e-14 and abs(math.exp(hi[10]) / g["prior_tref_hi"] - 1) < 1e-14
+    assert S.STRETCH_A == g["stretch_a"]
+
+
+def test_unpack_sampled_inverts_the_generator_transforms():
+    rng = np.random.default_rng(3)
+    p = np.stack([W.draw_prior(rng, 1e6, 3e7, q_range=(0.05, 1.0)) for _ in range(50)])
+    theta = p.copy()
+    theta[:, 0], theta[:, 4], theta[:, 10] = np.log(p[:, 0]), np.log(p[:, 4]), np.log(p[:, 10])
+    theta[:, 6], theta[:, 8] = np.cos(p[:, 6]), np.sin(p[:, 8])
+    assert np.all(S.in_prior(theta))
+    back = S.unpack_sampled(theta)
+    assert np.max(np.abs(back / p - 1.0)) < 1e-13
+    bad = theta[:3].copy()
+    bad[0, 1] = 1.2
+    bad[1, 6] = -1.0000001
+    bad[2, 10] = np.nan
+    assert not S.in_prior(bad).any()
+
+
+def test_philox_known_answers():
+    # Random123 known-answer vectors of philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11)
+    kat = [((0, 0, 0, 0), (0, 0), (0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8)),
+           ((0xffffffff,) * 4, (0xffffffff,) * 2, (0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd)),
+           ((0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344), (0xa4093822, 0x299f31d0), (0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1))]
+    for ctr, key, want in kat:
+        got = S.philox4x32(np.array(ctr, dtype=np.uint32), np.array(key, dtype=np.uint32))
+        assert tuple(int(x) for x in got) == want
+    u0, u1 = S.uniforms(12345, 7, 1, np.arange(100000))
+    assert 0.0 < u0.min() and u0.max() < 1.0 and abs(u0.mean() - 0.5) < 5e-3 and abs(np.corrcoef(u0, u1)[0, 1]) < 1e-2
+
+
+def test_stretch_z_has_the_density_of_eq_15():
+    a = S.STRETCH_A
+    u = np.linspace(0.0, 1.0, 1001)
+    z = S.stretch_z(u)
+    assert z[0] == 1.0 / a and abs(z[-1] - a) < 1e-15
+    cdf = (np.sqrt(z) - 1.0 / math.sqrt(a)) / (math.sqrt(a) - 1.0 / math.sqrt(a))      # integral of z^(-1/2) normalised on [1/a, a]
+    assert np.max(np.abs(cdf - u)) < 1e-14
+
+
+def test_stretch_move_and_swaps_sample_a_tempered_gaussian():
+    # detailed balance (eqs. 16, 17): a Gaussian likelihood inside the box must come out with variance sigma^2 / beta
+    mu = 0.5 * (S.PRIOR_LO + S.PRIOR_HI)
+    sig = 0.01 * (S.PRIOR_HI - S.PRIOR_LO)
+    fn = lambda th: -0.5 * np.sum(((th - mu) / sig) ** 2, axis=-1)
+    betas = np.array([1.0, 0.5, 0.25])
+    T, K = 3, 48
+    rng = np.random.default_rng(11)
+    theta = mu + sig * rng.standard_normal((T, K, 11)) / np.sqrt(betas)[:, None, None]
+    logl = fn(theta)
+    acc, samples = [], []
+    for step in range(1500):
+        for half in (0, 1):
+            theta, logl, a = S.stretch_half_step(theta, logl, betas, half, seed=99, step=2 * step + half, loglike_fn=fn)
+            acc.append(a.mean() * 2)
+        theta, logl, _ = S.swap_step(theta, logl, betas, seed=99, step=step)
+        if step >= 300:
+            samples.append(theta.copy())
+    assert np.allclose(logl, fn(theta), rtol=0, atol=1e-9)                      # bookkeeping of logl through moves and swaps
+    s = np.stack(samples)                                                        # [steps, T, K, 11]
+    for t in range(T):
+        x = (s[:, t] - mu) / sig
+        assert np.max(np.abs(x.mean(axis=(0, 1)))) < 0.15 / math.sqrt(betas[t])
+        ratio = x.var(axis=(0, 1)) * betas[t]
+        assert np.all(np.abs(ratio - 1.0) < 0.15), (t, ratio)
+    assert 0.2 < np.mean(acc) < 0.95
+
+
+def test_mode_products_are_linear_in_the_modes(table):
+    tf = lambda p, f, Sp: L.template(table, p, f, Sp)
+    wl = W.build(0, tf, n_bins=4096, batch=2)
+    p = wl["params"][1]
+    dh, hh = L.mode_products(table, p, wl["freqs"], wl["data"], wl["psd"], wl["S"])
+    tdh, thh, _ = L.loglike_parts(table, p, wl["freqs"], wl["data"], wl["psd"], wl["S"])
+    assert abs(dh.sum() - tdh) <= 1e-12 * (np.abs(dh).sum() + abs(tdh))        # <d|h> is linear in h
+    assert np.all(hh >= 0.0) and hh[0] == hh.max()                               # (2,2) dominates
+    assert thh <= np.sum(np.sqrt(hh)) ** 2 * (1 + 1e-12)                         # triangle inequality
+    assert abs(thh - hh.sum()) > 1e-6 * thh                                      # modes mix
