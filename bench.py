@@ -255,6 +255,62 @@ def run_dense_sweep(args):
         M.mbhl_free(ctx)
 
 
+def run_sampler(args):
+    """the parallel-tempered stretch-move ensemble of PAPER.md:193-222 driving the likelihood on
+    the device.  10 rungs (geometric ladder of base 2.04807, last rung at infinite temperature, :220-222) x 32 walkers
+    (4 walkers for each of the 8 sky modes per temperature, :222) around the 1e6 Msun injection of the config-2 data."""
+    torch, M, dev, local = _device_setup()
+    from paper_2005_01827_b200 import workloads as W
+    state = {}
+
+    def gpu_template(p, f, S):
+        if "ctx0" not in state:
+            n = f.size
+            state["ctx0"] = M.mbhl_init(torch.as_tensor(f, device=dev), torch.zeros((3, n, 2), dtype=torch.float64, device=dev),
+                                        torch.ones((3, n), dtype=torch.float64, device=dev), sparse_points=S, device=local)
+        h = M.mbhl_template(state["ctx0"], torch.as_tensor(p[None, :].copy(), device=dev))
+        torch.cuda.synchronize()
+        return h[0].cpu().numpy()
+
+    wl = W.build(2, gpu_template)
+    M.mbhl_free(state.pop("ctx0"))
+    t = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=dev)
+    T, K = 10, 32
+    ctx = M.mbhl_init(t(wl["freqs"]), t(wl["data"]), t(wl["psd"]), sparse_points=wl["S"], t0=wl["t0"], max_batch=T * K, device=local)
+    betas = 2.04807 ** -np.arange(T, dtype=np.float64)
+    betas[-1] = 0.0
+    inj = wl["injections"][1]
+    th0 = inj.copy()
+    th0[0], th0[4], th0[10] = np.log(inj[0]), np.log(inj[4]), np.log(inj[10])
+    th0[1] = 1.0 / inj[1] if inj[1] > 1.0 else inj[1]
+    th0[6], th0[8] = np.cos(inj[6]), np.sin(inj[8])
+    rng = np.random.default_rng(W.SEED0 + 5)
+    theta = th0 + np.array([1e-5, 1e-4, 1e-4, 1e-4, 1e-3, 1e-3, 1e-3, 1e-3, 1e-3, 1e-3, 1e-7]) * rng.standard_normal((T, K, 11))
+    pt = M.mbhl_pt_init(ctx, t(theta), betas, seed=W.SEED0, stretch_a=1.15)
+    M.mbhl_pt_step(pt, max(args.warmup, 3))
+    torch.cuda.synchronize()
+    launches0 = M.mbhl_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    M.mbhl_pt_step(pt, args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = M.mbhl_launch_count(ctx) - launches0
+    th, ll, acc, swp = M.mbhl_pt_state(pt, T, K, dev)
+    steps_done = max(args.warmup, 3) + args.steps
+    print(json.dumps({
+        "metric": "log-likelihoods/sec through the parallel-tempered ensemble", "value": T * K / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"PT ensemble {T} rungs x {K} walkers (two half-ensemble stretch moves of {T * K // 2} proposals + one swap sweep per step) "
+                               f"on the BASELINE.json configs[2] data (N={wl['freqs'].size}, S={wl['S']}), walkers around the 1e6 Msun injection"},
+        "gpu_launches": int(launches), "finite": bool(torch.isfinite(ll).all().item()),
+        "acceptance_per_rung": [float(a) / (steps_done * K) for a in acc],
+        "swap_fraction_per_pair": [float(x) / (steps_done * K) for x in swp]}))
+    M.mbhl_pt_free(pt)
+    M.mbhl_free(ctx)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -413,6 +469,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(0, 1, 2, 3, 4),
                     help="BASELINE.json config; 0-2 are likelihood workloads (2 = default bench line), 3 = sparse-stage isolation, "
                          "4 = dense N x B sweep (one JSON line per point)")
+    ap.add_argument("--sampler", action="store_true", help="time the parallel-tempered stretch-move ensemble (SURVEY 8(f).2) on the config-2 data")
     ap.add_argument("--batch", type=int, default=0, help="config 3 only: number of parameter sets (default 16384)")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
@@ -421,6 +478,8 @@ def main():
         if args.config > 2:
             raise SystemExit("--impl reference times the likelihood configs 0-2")
         run_reference(args)
+    elif args.sampler:
+        run_sampler(args)
     elif args.config == 3:
         run_sparse_isolation(args)
     elif args.config == 4:

@@ -112,6 +112,38 @@ size_t mbhl_workspace_bytes(const mbhl_ctx* ctx, int64_t B);
  * device allocation in the hot path and returns MBHL_ENOWS if it is too small.  NULL returns to internal.*/
 int mbhl_set_workspace(mbhl_ctx* ctx, void* dev_ptr, size_t bytes);
 
+/* ---- Sampler-side steps next to the likelihood (section II.B) -------------------- */
+
+/* Per-mode inner products (Table III :292-300): every mode evaluated in isolation against the
+ * data.  d_h[B][6] = <d|h_lm>, h_h[B][6] = <h_lm|h_lm> (optimal SNR of the mode alone = sqrt);
+ * either may be NULL.  Device pointers; mode order as above; a mode disabled at init gives 0.  B <= 65535.  */
+int mbhl_mode_products(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h);
+
+/* logL for walkers given in the sampler's coordinates (Table I :67-81)
+ *   theta[b] = (ln M_T, q, a1, a2, ln D_L, phi_ref, cos iota, lambda, sin beta, psi, ln t_ref),
+ * every component uniform between the bounds of Table I.  A walker outside that box gets logL = -inf (zero prior).
+ * theta, logL: device pointers.                                                                              */
+int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* logL);
+
+/* Parallel-tempered affine-invariant ensemble: n_temps rungs with inverse temperatures
+ * betas[t] (host pointer; beta = 0 is T = infinity, :222), n_walkers (even) walkers per rung in the sampler's
+ * coordinates, theta0[n_temps][n_walkers][11] (host or device pointer, copied).  One step = for each half of the
+ * ensemble a stretch move of every walker of that half against a partner drawn from the other half of its
+ * rung (eqs. 14-16 with parameter stretch_a, 1.15 in the paper) - the proposals of all rungs go through the
+ * likelihood hot path as ONE batch - then one sweep of swaps between adjacent rungs from the hottest pair
+ * down (eq. 17).  The target of rung t is prior x L^beta_t with the uniform prior of Table I (:211).  Random
+ * numbers: Philox4x32-10 keyed by seed, counter (walker, step, stream), so a run is reproducible.  The
+ * ensemble lives on the context's device and stream; nothing returns to the host between steps.
+ * n_temps * n_walkers <= 65535.  The context must outlive the ensemble.                                    */
+typedef struct mbhl_pt mbhl_pt;
+int  mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const double* betas, int32_t n_temps,
+                  int32_t n_walkers, uint64_t seed, double stretch_a);
+int  mbhl_pt_step(mbhl_pt* pt, int32_t n_steps);                  /* asynchronous on the context's stream   */
+/* Copies the ensemble out and synchronises: theta[n_temps][n_walkers][11], logL[n_temps][n_walkers] (host or
+ * device), accepted moves per rung n_accept[n_temps] and accepted swaps n_swap[n_temps-1] (host).  Any may be NULL. */
+int  mbhl_pt_state(mbhl_pt* pt, double* theta, double* logL, int64_t* n_accept, int64_t* n_swap);
+void mbhl_pt_free(mbhl_pt* pt);
+
 /* Introspection. */
 double  mbhl_data_norm(const mbhl_ctx* ctx);        /* <d|d> computed at init                            */
 int64_t mbhl_num_bins(const mbhl_ctx* ctx);

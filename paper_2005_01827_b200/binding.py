@@ -13,7 +13,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
-SYMBOLS = ("mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
+SYMBOLS = ("mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
+           "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
            "mbhl_launch_count", "mbhl_last_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
 
@@ -43,6 +44,13 @@ def lib():
         L.mbhl_loglike_parts.argtypes = [vp, vp, i64, vp, vp, vp]
         L.mbhl_loglike_host.argtypes = [vp, vp, i64, vp]
         L.mbhl_template.argtypes = [vp, vp, i64, vp, i64, vp, i32]
+        L.mbhl_mode_products.argtypes = [vp, vp, i64, vp, vp]
+        L.mbhl_loglike_sampled.argtypes = [vp, vp, i64, vp]
+        L.mbhl_pt_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32, i32, ctypes.c_uint64, dbl]
+        L.mbhl_pt_step.argtypes = [vp, i32]
+        L.mbhl_pt_state.argtypes = [vp, vp, vp, vp, vp]
+        L.mbhl_pt_free.argtypes = [vp]
+        L.mbhl_pt_free.restype = None
         L.mbhl_sparse.argtypes = [vp, vp, i64, vp, vp, vp]
         L.mbhl_workspace_bytes.argtypes = [vp, i64]
         L.mbhl_workspace_bytes.restype = ctypes.c_size_t
@@ -189,3 +197,47 @@ def mbhl_stage_times(ctx):
 
 def mbhl_dfma_probe(blocks, threads, iters, sink, stream=None):
     _check(lib().mbhl_dfma_probe(_stream_handle(stream), int(blocks), int(threads), int(iters), _ptr(sink)))
+
+
+def mbhl_mode_products(ctx, params):
+    """(<d|h_lm>, <h_lm|h_lm>) of every mode in isolation: two [B, 6] tensors."""
+    B = int(params.shape[0])
+    out = torch.empty((2, B, NMODE), dtype=torch.float64, device=params.device)
+    _check(lib().mbhl_mode_products(ctx, _ptr(params), B, _ptr(out[0]), _ptr(out[1])), ctx)
+    return out[0], out[1]
+
+
+def mbhl_loglike_sampled(ctx, theta, logL=None):
+    B = int(theta.shape[0])
+    if logL is None:
+        logL = torch.empty(B, dtype=torch.float64, device=theta.device)
+    _check(lib().mbhl_loglike_sampled(ctx, _ptr(theta), B, _ptr(logL)), ctx)
+    return logL
+
+
+def mbhl_pt_init(ctx, theta0, betas, seed=0, stretch_a=1.15):
+    """theta0 [T, K, 11] (torch CUDA or numpy), betas [T] numpy/host.  Returns the ensemble handle."""
+    T, K = int(theta0.shape[0]), int(theta0.shape[1])
+    betas = np.ascontiguousarray(betas, dtype=np.float64)
+    assert betas.shape == (T,)
+    pt = ctypes.c_void_p()
+    _check(lib().mbhl_pt_init(ctx, ctypes.byref(pt), _ptr(theta0), _ptr(betas), T, K, ctypes.c_uint64(int(seed)), float(stretch_a)), ctx)
+    return pt
+
+
+def mbhl_pt_step(pt, n_steps=1):
+    _check(lib().mbhl_pt_step(pt, int(n_steps)))
+
+
+def mbhl_pt_state(pt, T, K, device):
+    """Returns (theta [T,K,11], logL [T,K]) as torch tensors on `device` and (n_accept [T], n_swap [T-1]) as numpy."""
+    theta = torch.empty((T, K, NPARAM), dtype=torch.float64, device=device)
+    logl = torch.empty((T, K), dtype=torch.float64, device=device)
+    acc = np.zeros(T, dtype=np.int64)
+    swp = np.zeros(max(T - 1, 1), dtype=np.int64)
+    _check(lib().mbhl_pt_state(pt, _ptr(theta), _ptr(logl), ctypes.c_void_p(acc.ctypes.data), ctypes.c_void_p(swp.ctypes.data)))
+    return theta, logl, acc, swp[:T - 1]
+
+
+def mbhl_pt_free(pt):
+    lib().mbhl_pt_free(pt)

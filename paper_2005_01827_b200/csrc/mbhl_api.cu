@@ -163,6 +163,37 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     return MBHL_OK;
 }
 
+// Fused dense kernel + final reduction for the sparse stage results sitting in the workspace.
+int run_dense(mbhl_ctx* ctx, int64_t B, char* base, const WsLayout& L, uint32_t mode_mask, double* d_h, double* h_h, double* logL,
+              int64_t stride, bool count_work) {
+    const DensePlan P = dense_plan(B, n_chunks_of(ctx->N));
+    DenseArgs A;
+    A.dw = (const DenseWalker*)(base + L.dense);
+    A.knots = (const double*)(base + L.knots);
+    A.coef = (const double*)(base + L.coef);
+    A.tiles = ctx->tiles;
+    A.partials = (double*)(base + L.partials);
+    A.B = (int)B;
+    A.S = ctx->S;
+    A.W = P.W;
+    A.G = P.G;
+    A.n_chunks = n_chunks_of(ctx->N);
+    A.n_groups = P.n_groups;
+    A.inv_df = 1.0 / ctx->df;
+    A.mode_mask = mode_mask;
+    if (count_work) CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    const bool tm = ctx->timing && count_work;
+    if (tm) cudaEventRecord(ctx->ev[3], ctx->stream);
+    k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);
+    if (tm) cudaEventRecord(ctx->ev[4], ctx->stream);
+    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
+                                                                    count_work ? ctx->counters : nullptr, stride);
+    if (tm) { cudaEventRecord(ctx->ev[5], ctx->stream); ctx->n_timed += 1; }
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -226,6 +257,13 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     if (spline_smem_bytes(ctx->S) > 227 * 1024) return cleanup(MBHL_EINVAL);   // S <= ~2170 fits one CTA's shared memory
     if (cudaSetDevice(ctx->device) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
+    {
+        // Table I: ln M_T, q, a1, a2, ln D_L, phi_ref, cos iota, lambda, sin beta, psi, ln t_ref
+        const double lo[MBHL_NPARAM] = {log(1e3), 0.05, -0.99, -0.99, log(0.044), 0.0, -1.0, 0.0, -1.0, 0.0, log(1.0)};
+        const double hi[MBHL_NPARAM] = {log(1e9), 1.0, 0.99, 0.99, log(1298.00), 2.0 * M_PI, 1.0, 2.0 * M_PI, 1.0, M_PI, log(3.15576e8)};
+        if (cudaMemcpyToSymbol(c_prior_lo, lo, sizeof(lo)) != cudaSuccess || cudaMemcpyToSymbol(c_prior_hi, hi, sizeof(hi)) != cudaSuccess)
+            return cleanup(MBHL_ECUDA);
+    }
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
@@ -342,29 +380,8 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     const WsLayout L = layout(ctx, B);
     rc = run_sparse(ctx, params, B, base, L, true);
     if (rc != MBHL_OK) return rc;
-    const DensePlan P = dense_plan(B, n_chunks_of(ctx->N));
-    DenseArgs A;
-    A.dw = (const DenseWalker*)(base + L.dense);
-    A.knots = (const double*)(base + L.knots);
-    A.coef = (const double*)(base + L.coef);
-    A.tiles = ctx->tiles;
-    A.partials = (double*)(base + L.partials);
-    A.B = (int)B;
-    A.S = ctx->S;
-    A.W = P.W;
-    A.G = P.G;
-    A.n_chunks = n_chunks_of(ctx->N);
-    A.n_groups = P.n_groups;
-    A.inv_df = 1.0 / ctx->df;
-    CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
-    if (ctx->timing) cudaEventRecord(ctx->ev[3], ctx->stream);
-    k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);
-    if (ctx->timing) cudaEventRecord(ctx->ev[4], ctx->stream);
-    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
-                                                                    ctx->counters);
-    if (ctx->timing) { cudaEventRecord(ctx->ev[5], ctx->stream); ctx->n_timed += 1; }
-    ctx->launches += 2;
-    CU(cudaGetLastError());
+    rc = run_dense(ctx, B, base, L, ctx->mode_mask, d_h, h_h, logL, 1, true);
+    if (rc != MBHL_OK) return rc;
     return MBHL_OK;
 }
 
@@ -390,6 +407,143 @@ int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, doubl
     CU(cudaMemcpyAsync(logL_host, l_dev, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MBHL_OK;
+}
+
+int mbhl_mode_products(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || B > 65535 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B (B <= 65535)");
+    if (B == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    const bool tm = ctx->timing;
+    ctx->timing = false;
+    rc = run_sparse(ctx, params, B, base, L, true);
+    for (int mi = 0; mi < MBHL_NMODE && rc == MBHL_OK; ++mi)
+        rc = run_dense(ctx, B, base, L, ctx->mode_mask & (1u << mi), d_h ? d_h + mi : nullptr, h_h ? h_h + mi : nullptr, nullptr,
+                       MBHL_NMODE, false);
+    ctx->timing = tm;
+    return rc;
+}
+
+int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* logL) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && (!theta || !logL))) return fail(ctx, MBHL_EINVAL, "bad theta/logL/B");
+    if (B == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    char* base;
+    int rc = get_workspace(ctx, B, &base);
+    if (rc != MBHL_OK) return rc;
+    const WsLayout L = layout(ctx, B);
+    double* p_dev = (double*)(base + L.params);
+    k_unpack_sampled<<<(unsigned)((B + 127) / 128), 128, 0, ctx->stream>>>(theta, B, p_dev);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return mbhl_loglike_parts(ctx, p_dev, B, nullptr, nullptr, logL);
+}
+
+// ---------------------------------------------------------------------------------------------
+// parallel-tempered stretch-move ensemble driving the likelihood on the device
+// ---------------------------------------------------------------------------------------------
+struct mbhl_pt {
+    mbhl_ctx* ctx = nullptr;
+    PtState s = {};
+    void* mem = nullptr;
+    uint32_t step = 0;
+};
+
+int mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const double* betas_host, int32_t n_temps,
+                 int32_t n_walkers, uint64_t seed, double stretch_a) {
+    if (!ctx || !out) return MBHL_EINVAL;
+    *out = nullptr;
+    if (!theta0 || !betas_host || n_temps < 1 || n_walkers < 2 || (n_walkers & 1) || !(stretch_a > 1.0) ||
+        (int64_t)n_temps * n_walkers > 65535)
+        return fail(ctx, MBHL_EINVAL, "mbhl_pt_init: need n_temps >= 1, an even n_walkers >= 2, n_temps * n_walkers <= 65535, a > 1");
+    for (int t = 0; t < n_temps; ++t)
+        if (!(betas_host[t] >= 0.0) || !isfinite(betas_host[t])) return fail(ctx, MBHL_EINVAL, "mbhl_pt_init: betas must be finite and >= 0");
+    CU(cudaSetDevice(ctx->device));
+    mbhl_pt* pt = new (std::nothrow) mbhl_pt();
+    if (!pt) return MBHL_ENOMEM;
+    pt->ctx = ctx;
+    const size_t T = (size_t)n_temps, K = (size_t)n_walkers, H = K / 2;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align256(bytes); return o; };
+    const size_t o_theta = take(T * K * MBHL_NPARAM * 8), o_logl = take(T * K * 8), o_betas = take(T * 8);
+    const size_t o_pth = take(T * H * MBHL_NPARAM * 8), o_ppar = take(T * H * MBHL_NPARAM * 8), o_pl = take(T * H * 8), o_pz = take(T * H * 8);
+    const size_t o_acc = take(T * 8), o_swp = take(T * 8), o_tmp = take(T * K * MBHL_NPARAM * 8);
+    if (cudaMalloc(&pt->mem, off) != cudaSuccess) {
+        cudaGetLastError();
+        delete pt;
+        return fail(ctx, MBHL_ENOMEM, "mbhl_pt_init: cudaMalloc");
+    }
+    char* m = (char*)pt->mem;
+    PtState& s = pt->s;
+    s.theta = (double*)(m + o_theta); s.logl = (double*)(m + o_logl); s.betas = (double*)(m + o_betas);
+    s.prop_theta = (double*)(m + o_pth); s.prop_params = (double*)(m + o_ppar); s.prop_logl = (double*)(m + o_pl);
+    s.prop_z = (double*)(m + o_pz); s.n_accept = (unsigned long long*)(m + o_acc); s.n_swap = (unsigned long long*)(m + o_swp);
+    s.T = n_temps; s.K = n_walkers; s.a = stretch_a; s.seed = seed;
+    int rc = MBHL_OK;
+    auto bail = [&](int code) { cudaFree(pt->mem); delete pt; return code; };
+    if (cudaMemcpyAsync(s.theta, theta0, T * K * MBHL_NPARAM * 8, cudaMemcpyDefault, ctx->stream) != cudaSuccess ||
+        cudaMemcpyAsync(s.betas, betas_host, T * 8, cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
+        cudaMemsetAsync(s.n_accept, 0, 2 * align256(T * 8), ctx->stream) != cudaSuccess)
+        return bail(fail(ctx, MBHL_ECUDA, "mbhl_pt_init: copies"));
+    // log-likelihood of the starting positions (walkers outside the prior box get -inf)
+    double* tmp = (double*)(m + o_tmp);
+    k_unpack_sampled<<<(unsigned)((T * K + 127) / 128), 128, 0, ctx->stream>>>(s.theta, (int64_t)(T * K), tmp);
+    ctx->launches += 1;
+    rc = mbhl_loglike_parts(ctx, tmp, (int64_t)(T * K), nullptr, nullptr, s.logl);
+    if (rc != MBHL_OK) return bail(rc);
+    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return bail(fail(ctx, MBHL_ECUDA, "mbhl_pt_init: sync"));
+    *out = pt;
+    return MBHL_OK;
+}
+
+int mbhl_pt_step(mbhl_pt* pt, int32_t n_steps) {
+    if (!pt || n_steps < 0) return MBHL_EINVAL;
+    mbhl_ctx* ctx = pt->ctx;
+    CU(cudaSetDevice(ctx->device));
+    const PtState& s = pt->s;
+    const int M = s.T * (s.K / 2);
+    for (int it = 0; it < n_steps; ++it, ++pt->step) {
+        for (int half = 0; half < 2; ++half) {
+            k_pt_propose<<<(M + 127) / 128, 128, 0, ctx->stream>>>(s, half, 2u * pt->step + (uint32_t)half);
+            int rc = mbhl_loglike_parts(ctx, s.prop_params, M, nullptr, nullptr, s.prop_logl);
+            if (rc != MBHL_OK) return rc;
+            k_pt_accept<<<(M + 127) / 128, 128, 0, ctx->stream>>>(s, half, 2u * pt->step + (uint32_t)half);
+            ctx->launches += 2;
+        }
+        if (s.T > 1) {
+            k_pt_swap<<<(s.K + 127) / 128, 128, 0, ctx->stream>>>(s, pt->step);
+            ctx->launches += 1;
+        }
+    }
+    CU(cudaGetLastError());
+    return MBHL_OK;
+}
+
+int mbhl_pt_state(mbhl_pt* pt, double* theta, double* logL, int64_t* n_accept_host, int64_t* n_swap_host) {
+    if (!pt) return MBHL_EINVAL;
+    mbhl_ctx* ctx = pt->ctx;
+    CU(cudaSetDevice(ctx->device));
+    const PtState& s = pt->s;
+    const size_t n = (size_t)s.T * s.K;
+    if (theta) CU(cudaMemcpyAsync(theta, s.theta, n * MBHL_NPARAM * 8, cudaMemcpyDefault, ctx->stream));
+    if (logL) CU(cudaMemcpyAsync(logL, s.logl, n * 8, cudaMemcpyDefault, ctx->stream));
+    if (n_accept_host) CU(cudaMemcpyAsync(n_accept_host, s.n_accept, (size_t)s.T * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    if (n_swap_host && s.T > 1) CU(cudaMemcpyAsync(n_swap_host, s.n_swap, (size_t)(s.T - 1) * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MBHL_OK;
+}
+
+void mbhl_pt_free(mbhl_pt* pt) {
+    if (!pt) return;
+    cudaSetDevice(pt->ctx->device);
+    cudaStreamSynchronize(pt->ctx->stream);
+    cudaFree(pt->mem);
+    delete pt;
 }
 
 int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins) {

@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
     const bool p_own = tid < nb * MBHL_NMODE;
     DenseMode p_m;
     p_m.k_lo = 1; p_m.k_hi = 0; p_m.ln_flo = 0.0; p_m.inv_dlog = 0.0;
-    if (p_own && s_dw[p_wi].valid) p_m = s_dw[p_wi].mode[p_mi];
+    if (p_own && s_dw[p_wi].valid && ((A.mode_mask >> p_mi) & 1u)) p_m = s_dw[p_wi].mode[p_mi];
     if (p_m.k_hi >= p_m.k_lo) { atomicMin(&s_range[0], p_m.k_lo); atomicMax(&s_range[1], p_m.k_hi); }
     const double* const p_x = A.knots + ((int64_t)(b0 + p_wi) * MBHL_NMODE + p_mi) * A.S;
     const double* const p_coef = A.coef + ((int64_t)(b0 + p_wi) * MBHL_NMODE + p_mi) * (int64_t)(A.S - 1) * kCoefStride;

@@ -392,6 +392,7 @@ struct DenseArgs {
     int n_chunks;
     int n_groups;
     double inv_df;           // 1 / bin spacing of the init grid
+    uint32_t mode_mask;      // modes evaluated by this launch (bit i = mode i); the others count as out of band
 };
 
 // sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
@@ -481,6 +482,7 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
 }  // namespace mbhl
 
 #include "mbhl_dense.cuh"   // a6 + a7: the fused dense kernel
+#include "mbhl_sampler.cuh" // sampler coordinates, stretch move, temperature swaps
 
 namespace mbhl {
 
@@ -488,7 +490,7 @@ namespace mbhl {
 __global__ void __launch_bounds__(128) k_final_reduce(const DenseWalker* __restrict__ dw, const double* __restrict__ partials,
                                                       int n_groups, int64_t B, double dd, double* __restrict__ d_h,
                                                       double* __restrict__ h_h, double* __restrict__ logL,
-                                                      unsigned long long* __restrict__ counters) {
+                                                      unsigned long long* __restrict__ counters, int64_t stride) {
     const int64_t b = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (b >= B) return;
     const int lane = threadIdx.x & 31;
@@ -503,10 +505,10 @@ __global__ void __launch_bounds__(128) k_final_reduce(const DenseWalker* __restr
     if (lane == 0) {
         const bool valid = dw[b].valid != 0;
         if (!valid) { sdh = 0.0; shh = 0.0; }
-        if (d_h) d_h[b] = sdh;
-        if (h_h) h_h[b] = shh;
-        if (logL) logL[b] = valid ? (sdh - 0.5 * shh - 0.5 * dd) : -INFINITY;
-        if (valid && dw[b].pairs) {
+        if (d_h) d_h[b * stride] = sdh;
+        if (h_h) h_h[b * stride] = shh;
+        if (logL) logL[b * stride] = valid ? (sdh - 0.5 * shh - 0.5 * dd) : -INFINITY;
+        if (counters && valid && dw[b].pairs) {
             atomicAdd(counters, (unsigned long long)dw[b].pairs);
             atomicAdd(counters + 1, (unsigned long long)dw[b].bins);
         }

@@ -1,0 +1,163 @@
+// mbhl_sampler.cuh - sampler-side steps next to the likelihood (section II.B).
+//
+//   k_unpack_sampled   sampler coordinates (Table I :67-81) -> physical parameters;
+//                      a walker outside the prior box becomes a NaN row, which the hot path maps to logL = -inf
+//   k_pt_propose       stretch move, eqs. 14-15, a = 1.15 (:222): one thread per moving walker
+//   k_pt_accept        eq. 16 on the tempered density prior x L^beta (:211)
+//   k_pt_swap          eq. 17: swaps between adjacent temperatures, hottest pair first
+// Random numbers come from Philox4x32-10 (Salmon et al. 2011) keyed by the seed and counted by (walker, step,
+// stream), so a run is reproducible and independent of the launch shape.  Written from the paper and the
+// generator's published definition; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mbhl {
+
+// Table I; filled by mbhl_init from the host's log() of the printed bounds
+__constant__ double c_prior_lo[MBHL_NPARAM];
+__constant__ double c_prior_hi[MBHL_NPARAM];
+
+__device__ __forceinline__ bool in_prior_box(const double* th) {
+    bool ok = true;
+#pragma unroll
+    for (int i = 0; i < MBHL_NPARAM; ++i) ok = ok && isfinite(th[i]) && th[i] >= c_prior_lo[i] && th[i] <= c_prior_hi[i];
+    return ok;
+}
+
+// theta = (ln M_T, q, a1, a2, ln D_L, phi_ref, cos iota, lambda, sin beta, psi, ln t_ref)
+__device__ __forceinline__ void unpack_sampled(const double* th, double* p) {
+    if (!in_prior_box(th)) {
+#pragma unroll
+        for (int i = 0; i < MBHL_NPARAM; ++i) p[i] = NAN;
+        return;
+    }
+    p[0] = exp(th[0]); p[1] = th[1]; p[2] = th[2]; p[3] = th[3]; p[4] = exp(th[4]); p[5] = th[5];
+    p[6] = acos(th[6]); p[7] = th[7]; p[8] = asin(th[8]); p[9] = th[9]; p[10] = exp(th[10]);
+}
+
+__global__ void k_unpack_sampled(const double* __restrict__ theta, int64_t B, double* __restrict__ params) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    double th[MBHL_NPARAM], p[MBHL_NPARAM];
+#pragma unroll
+    for (int i = 0; i < MBHL_NPARAM; ++i) th[i] = theta[b * MBHL_NPARAM + i];
+    unpack_sampled(th, p);
+#pragma unroll
+    for (int i = 0; i < MBHL_NPARAM; ++i) params[b * MBHL_NPARAM + i] = p[i];
+}
+
+// Philox4x32-10: counter c[4], key k[2]
+__device__ __forceinline__ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c[0]), lo0 = 0xD2511F53u * c[0];
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c[2]), lo1 = 0xCD9E8D57u * c[2];
+        const uint32_t n0 = hi1 ^ c[1] ^ k0, n2 = hi0 ^ c[3] ^ k1;
+        c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+}
+
+// two uniforms in (0, 1), 52 random bits each: counter = (index, step, stream, 0), key = seed
+__device__ __forceinline__ void uniforms2(uint64_t seed, uint32_t step, uint32_t stream, uint32_t index, double& u0, double& u1) {
+    uint32_t c[4] = {index, step, stream, 0u};
+    philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+    const uint64_t a = ((uint64_t)c[0] << 20) | (c[1] >> 12), b = ((uint64_t)c[2] << 20) | (c[3] >> 12);
+    u0 = ((double)a + 0.5) * 0x1p-52;
+    u1 = ((double)b + 0.5) * 0x1p-52;
+}
+
+struct PtState {
+    double* theta;       // [T][K][11] sampler coordinates
+    double* logl;        // [T][K]
+    double* betas;       // [T]
+    double* prop_theta;  // [T][K/2][11] proposals (sampler coordinates)
+    double* prop_params; // [T][K/2][11] proposals (physical, NaN rows outside the prior)
+    double* prop_logl;   // [T][K/2]
+    double* prop_z;      // [T][K/2]
+    unsigned long long* n_accept;   // [T]
+    unsigned long long* n_swap;     // [T-1]
+    int T, K;
+    double a;            // stretch parameter
+    uint64_t seed;
+};
+
+// Walkers k with k % 2 == half move; moving walker number i of temperature t is k = 2 i + half.
+__global__ void k_pt_propose(PtState s, int half, uint32_t step) {
+    const int hk = s.K / 2;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= s.T * hk) return;
+    const int t = idx / hk, i = idx - t * hk;
+    const int k = 2 * i + half;
+    double u_z, u_j;
+    uniforms2(s.seed, step, 0u, (uint32_t)(t * s.K + k), u_z, u_j);
+    const double g = __dadd_rn(__dmul_rn(s.a - 1.0, u_z), 1.0);
+    const double z = __ddiv_rn(__dmul_rn(g, g), s.a);                       // eq. 15 by inverting its CDF
+    int jj = (int)(u_j * hk);
+    jj = min(jj, hk - 1);
+    const int j = 2 * jj + (1 - half);                                       // partner from the other half
+    const double* xk = s.theta + ((int64_t)t * s.K + k) * MBHL_NPARAM;
+    const double* xj = s.theta + ((int64_t)t * s.K + j) * MBHL_NPARAM;
+    double y[MBHL_NPARAM], p[MBHL_NPARAM];
+#pragma unroll
+    for (int d = 0; d < MBHL_NPARAM; ++d) y[d] = __dadd_rn(xj[d], __dmul_rn(z, __dadd_rn(xk[d], -xj[d])));   // eq. 14, no contraction
+    unpack_sampled(y, p);
+#pragma unroll
+    for (int d = 0; d < MBHL_NPARAM; ++d) {
+        s.prop_theta[(int64_t)idx * MBHL_NPARAM + d] = y[d];
+        s.prop_params[(int64_t)idx * MBHL_NPARAM + d] = p[d];
+    }
+    s.prop_z[idx] = z;
+}
+
+__global__ void k_pt_accept(PtState s, int half, uint32_t step) {
+    const int hk = s.K / 2;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= s.T * hk) return;
+    const int t = idx / hk, i = idx - t * hk;
+    const int k = 2 * i + half;
+    const int64_t w = (int64_t)t * s.K + k;
+    double u, unused;
+    uniforms2(s.seed, step, 1u, (uint32_t)w, u, unused);
+    const double ln_new = s.prop_logl[idx], ln_old = s.logl[w], beta = s.betas[t];
+    // ln of eq. 16 on the tempered density: (D - 1) ln z + beta (ln L(Y) - ln L(X)); outside the prior box L(Y) = 0
+    bool acc = false;
+    if (isfinite(ln_new)) {
+        const double lnr = (MBHL_NPARAM - 1) * log(s.prop_z[idx]) + (beta * ln_new - beta * ln_old);
+        acc = log(u) < lnr;
+    }
+    if (acc) {
+#pragma unroll
+        for (int d = 0; d < MBHL_NPARAM; ++d) s.theta[w * MBHL_NPARAM + d] = s.prop_theta[(int64_t)idx * MBHL_NPARAM + d];
+        s.logl[w] = ln_new;
+        atomicAdd(s.n_accept + t, 1ULL);
+    }
+}
+
+// one thread per walker slot k: rung pairs (i, i-1) from the hottest down, as eq. 17
+__global__ void k_pt_swap(PtState s, uint32_t step) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= s.K) return;
+    for (int i = s.T - 1; i >= 1; --i) {
+        const int64_t wi = (int64_t)i * s.K + k, wj = (int64_t)(i - 1) * s.K + k;
+        double u, unused;
+        uniforms2(s.seed, step, 2u, (uint32_t)wi, u, unused);
+        const double li = s.logl[wi], lj = s.logl[wj];
+        const double lnr = (s.betas[i - 1] - s.betas[i]) * (li - lj);
+        if (log(u) < lnr) {
+#pragma unroll
+            for (int d = 0; d < MBHL_NPARAM; ++d) {
+                const double a = s.theta[wi * MBHL_NPARAM + d];
+                s.theta[wi * MBHL_NPARAM + d] = s.theta[wj * MBHL_NPARAM + d];
+                s.theta[wj * MBHL_NPARAM + d] = a;
+            }
+            s.logl[wi] = lj;
+            s.logl[wj] = li;
+            atomicAdd(s.n_swap + (i - 1), 1ULL);
+        }
+    }
+}
+
+}  // namespace mbhl

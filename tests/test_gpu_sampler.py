@@ -1,0 +1,124 @@
+"""GPU parity tests of the sampler-side calls: per-mode products, sampler coordinates,
+parallel-tempered stretch-move ensemble, each against oracle/ on the same seeded inputs."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import likelihood as L
+from oracle import sampler as S
+from paper_2005_01827_b200 import binding as M
+from paper_2005_01827_b200 import workloads as W
+
+DEV = "cuda:0"
+
+
+def dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x), device=DEV)
+
+
+def to_sampled(p):
+    """Physical parameters -> the sampler's coordinates; q is mapped into (0, 1] (q and 1/q are the same binary, G15)."""
+    th = np.array(p, dtype=np.float64, copy=True)
+    th[..., 0], th[..., 4], th[..., 10] = np.log(p[..., 0]), np.log(p[..., 4]), np.log(p[..., 10])
+    th[..., 1] = np.where(p[..., 1] > 1.0, 1.0 / p[..., 1], p[..., 1])
+    th[..., 6], th[..., 8] = np.cos(p[..., 6]), np.sin(p[..., 8])
+    return th
+
+
+@pytest.fixture(scope="module")
+def small(table):
+    wl = W.build(0, lambda p, f, Sp: L.template(table, p, f, Sp), n_bins=4096, batch=4)
+    wl["S"] = 64
+    return wl
+
+
+def make_ctx(wl):
+    return M.mbhl_init(dev(wl["freqs"]), dev(wl["data"]), dev(wl["psd"]), sparse_points=wl["S"], t0=wl["t0"])
+
+
+def test_mode_products_parity(table, small):
+    ctx = make_ctx(small)
+    p = small["params"]
+    dh, hh = [t.cpu().numpy() for t in M.mbhl_mode_products(ctx, dev(p))]
+    tdh, thh, _ = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(p))]
+    for b in range(p.shape[0]):
+        rdh, rhh = L.mode_products(table, p[b], small["freqs"], small["data"], small["psd"], small["S"], small["t0"])
+        assert np.all(np.abs(hh[b] - rhh) <= 1e-8 * rhh.max())
+        assert np.all(np.abs(dh[b] - rdh) <= 1e-8 * max(np.abs(rdh).max(), rhh.max()))
+        assert abs(dh[b].sum() - tdh[b]) <= 1e-10 * (np.abs(dh[b]).sum() + abs(tdh[b]))       # <d|h> is linear over the modes
+    # a mode disabled at init gives zero
+    ctx2 = M.mbhl_init(dev(small["freqs"]), dev(small["data"]), dev(small["psd"]), sparse_points=small["S"], mode_mask=0b000101)
+    dh2, hh2 = [t.cpu().numpy() for t in M.mbhl_mode_products(ctx2, dev(p))]
+    assert np.all(hh2[:, [1, 3, 4, 5]] == 0.0) and np.all(dh2[:, [1, 3, 4, 5]] == 0.0)
+    assert np.allclose(hh2[:, [0, 2]], hh[:, [0, 2]], rtol=1e-13, atol=0.0)
+    M.mbhl_free(ctx)
+    M.mbhl_free(ctx2)
+
+
+def test_loglike_sampled_parity(table, small):
+    ctx = make_ctx(small)
+    p = small["params"]
+    th = to_sampled(p)
+    assert np.all(S.in_prior(th))
+    ll = M.mbhl_loglike_sampled(ctx, dev(th)).cpu().numpy()
+    for b in range(p.shape[0]):
+        ref = L.loglike_parts(table, S.unpack_sampled(th[b]), small["freqs"], small["data"], small["psd"], small["S"], small["t0"])[2]
+        assert abs(ll[b] - ref) <= 1e-6 * (1.0 + abs(ref)), (b, ll[b], ref)
+    bad = th.copy()
+    bad[0, 1] = 1.5                 # q outside Table I
+    bad[1, 6] = 1.0 + 1e-12         # cos(iota) > 1
+    bad[2, 0] = math.log(1e10)      # M_T above the box
+    bad[3, 10] = np.nan
+    out = M.mbhl_loglike_sampled(ctx, dev(bad)).cpu().numpy()
+    assert np.all(np.isneginf(out))
+    M.mbhl_free(ctx)
+
+
+def test_pt_ensemble_parity(table, small):
+    # T = 3 rungs (the last at infinite temperature), K = 8 walkers, a few steps: GPU ensemble against the oracle's
+    ctx = make_ctx(small)
+    T, K = 3, 8
+    betas = np.array([1.0, 0.4, 0.0])
+    rng = np.random.default_rng(5)
+    th0 = to_sampled(small["injections"][0])
+    width = np.array([1e-4, 1e-3, 1e-3, 1e-3, 1e-2, 1e-2, 1e-2, 1e-2, 1e-2, 1e-2, 1e-5])
+    theta = th0 + width * rng.standard_normal((T, K, 11))
+    theta[..., 1] = np.clip(theta[..., 1], 0.06, 0.999)
+    theta[..., 6] = np.clip(theta[..., 6], -0.999, 0.999)
+    theta[..., 8] = np.clip(theta[..., 8], -0.999, 0.999)
+    assert np.all(S.in_prior(theta))
+
+    def fn(th):
+        return np.array([L.loglike_parts(table, S.unpack_sampled(t), small["freqs"], small["data"], small["psd"], small["S"], small["t0"])[2]
+                         for t in th])
+
+    logl = fn(theta.reshape(-1, 11)).reshape(T, K)
+    pt = M.mbhl_pt_init(ctx, dev(theta), betas, seed=2005018270001, stretch_a=S.STRETCH_A)
+    g_theta, g_logl, _, _ = M.mbhl_pt_state(pt, T, K, DEV)
+    assert np.array_equal(g_theta.cpu().numpy(), theta)
+    assert np.max(np.abs(g_logl.cpu().numpy() - logl) / (1.0 + np.abs(logl))) <= 1e-6
+    n_acc = np.zeros(T, dtype=np.int64)
+    n_swp = np.zeros(T - 1, dtype=np.int64)
+    for step in range(5):
+        for half in (0, 1):
+            theta, logl, a = S.stretch_half_step(theta, logl, betas, half, 2005018270001, 2 * step + half, fn)
+            n_acc += a.sum(axis=1)
+        theta, logl, sw = S.swap_step(theta, logl, betas, 2005018270001, step)
+        n_swp += sw.sum(axis=1)
+        M.mbhl_pt_step(pt, 1)
+        g_theta, g_logl, g_acc, g_swp = M.mbhl_pt_state(pt, T, K, DEV)
+        assert np.max(np.abs(g_theta.cpu().numpy() - theta)) <= 1e-12, step
+        assert np.max(np.abs(g_logl.cpu().numpy() - logl) / (1.0 + np.abs(logl))) <= 1e-6, step
+        assert np.array_equal(g_acc, n_acc) and np.array_equal(g_swp, n_swp), step
+    assert n_acc.sum() > 0 and n_acc[-1] > 0          # the infinite-temperature rung accepts in-prior moves with z^(D-1)
+    M.mbhl_pt_free(pt)
+    # argument checks
+    with pytest.raises(M.MbhlError):
+        M.mbhl_pt_init(ctx, dev(theta[:, :7]), betas)          # odd number of walkers
+    with pytest.raises(M.MbhlError):
+        M.mbhl_pt_init(ctx, dev(theta), np.array([1.0, -0.5, 0.0]))
+    M.mbhl_free(ctx)
