@@ -600,9 +600,12 @@ int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, d
         k_export_y<<<(unsigned)((rows * ctx->S + 255) / 256), 256, 0, ctx->stream>>>((const double*)(base + L.y), rows, ctx->S, y);
         ctx->launches += 1;
     }
-    if (coef)
-        CU(cudaMemcpyAsync(coef, base + L.coef, (size_t)B * MBHL_NMODE * (ctx->S - 1) * kCoefStride * sizeof(double),
-                           cudaMemcpyDeviceToDevice, ctx->stream));
+    if (coef) {
+        const int64_t n = B * MBHL_NMODE * (int64_t)(ctx->S - 1) * MBHL_NQ;
+        k_export_coef<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>((const WalkerConst*)(base + L.consts), (const double*)(base + L.knots),
+                                                                           (const double*)(base + L.coef), B * MBHL_NMODE, ctx->S, coef);
+        ctx->launches += 1;
+    }
     CU(cudaGetLastError());
     return MBHL_OK;
 }

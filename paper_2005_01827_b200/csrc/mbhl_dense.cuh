@@ -1,4 +1,4 @@
-// mbhl_dense.cuh - steps a6 + a7: the fused dense kernel, version 3.
+// mbhl_dense.cuh - steps a6 + a7: the fused dense kernel, version 4.
 //
 // Interpolates every active mode onto the Fourier bins, sums the modes per bin and accumulates
 // <d|h> and <h|h> (eqs. 2, 3, 11).  The template is never written to memory (the paper
@@ -24,8 +24,10 @@
 // One partial per (walker, CTA) leaves the kernel; k_final_reduce adds them in fixed order (bitwise
 // reproducible, no atomics on values).
 //
-// The loop body is FP64-pipe bound: per (bin, mode) 8 Horner cubics (24 DFMA), the exact linear phase term
-// (reading G9), a quarter-turn sincos (19) and 3 complex multiply-adds (12).
+// The loop body is FP64-pipe bound: per (bin, mode) 8 Horner cubics (24 DFMA), a quarter-turn sincos (17) and
+// 3 complex multiply-adds (12).  The linear term -2 pi f t_coal of the phase (reading G9) costs nothing here:
+// k_spline folds it into the phase record of every interval (exact reduction of x_j t_coal, slope minus
+// t_coal), so the total phase of a bin in quarter turns is one cubic in u = f - x_j.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -87,7 +89,7 @@ __device__ __forceinline__ void sincos_qturn_x(const double (&p4)[kDenseR], doub
 // kGated: the amplitude of bin r is multiplied by gate[r] (1 inside the segment served by `rec`, else 0).
 template <bool kGated>
 __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, double xj, const double (&f)[kDenseR],
-                                             const double (&lin4)[kDenseR], const double (&gate)[kDenseR],
+                                             const double (&gate)[kDenseR],
                                              double (&h)[kDenseR][6]) {
     double u[kDenseR], are[kDenseR], aim[kDenseR];
 #pragma unroll
@@ -102,8 +104,6 @@ __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, dou
         for (int r = 0; r < kDenseR; ++r) p4[r] = fma(p4[r], u[r], p01.y);
 #pragma unroll
         for (int r = 0; r < kDenseR; ++r) p4[r] = fma(p4[r], u[r], p01.x);
-#pragma unroll
-        for (int r = 0; r < kDenseR; ++r) p4[r] = fma(p4[r], 4.0, -lin4[r]);
         sincos_qturn_x(p4, sn, cs);
         const double2 a01 = *reinterpret_cast<const double2*>(rec);
         const double2 a23 = *reinterpret_cast<const double2*>(rec + 2);
@@ -293,12 +293,10 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
             unsigned m_part = __ballot_sync(0xffffffffu, part);
             unsigned m_gen = __ballot_sync(0xffffffffu, gen);
             if (!(m_full | m_part | m_gen)) continue;
-            const double t_coal = s_dw[wi].t_coal;
 
-            double lin4[kDenseR], h[kDenseR][6];
+            double h[kDenseR][6];
 #pragma unroll
             for (int r = 0; r < kDenseR; ++r) {
-                lin4[r] = 4.0 * linear_cycles(f[r], t_coal);
 #pragma unroll
                 for (int i = 0; i < 6; ++i) h[r][i] = 0.0;
             }
@@ -306,7 +304,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                 const int mi = __ffs(m_full) - 1;
                 m_full &= m_full - 1;
                 const int slot = 2 * (wi * MBHL_NMODE + mi) + ((m_selB >> mi) & 1u);
-                mode_uniform<false>(s_rec + slot * kCoefStride, s_xj[slot], f, lin4, lin4, h);
+                mode_uniform<false>(s_rec + slot * kCoefStride, s_xj[slot], f, f, h);
             }
             while (m_part) {
                 // band edge or knot inside the warp tile: each staged segment is evaluated on all bins and gated
@@ -325,7 +323,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                         gate[r] = (o >= lo && o <= hi) ? 1.0 : 0.0;
                     }
                     const int slot = 2 * (wi * MBHL_NMODE + mi) + seg;
-                    mode_uniform<true>(s_rec + slot * kCoefStride, s_xj[slot], f, lin4, gate, h);
+                    mode_uniform<true>(s_rec + slot * kCoefStride, s_xj[slot], f, gate, h);
                 }
             }
             if (m_gen) {
@@ -351,7 +349,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                     const double* x = xk + mi * A.S;
                     const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
                     if (ja_m == jb_m && full_m) {
-                        mode_uniform<false>(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, lin4, lin4, h);
+                        mode_uniform<false>(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, f, h);
                     } else {
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
 #pragma unroll
@@ -361,7 +359,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                             int j = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
                             while (j > ja_m && f[r] < __ldg(x + j)) --j;
                             while (j < jb_m && f[r] >= __ldg(x + j + 1)) ++j;
-                            mode_contrib(cbase + (int64_t)j * kCoefStride, f[r] - __ldg(x + j), lin4[r], 1.0, h[r]);
+                            mode_contrib(cbase + (int64_t)j * kCoefStride, f[r] - __ldg(x + j), 1.0, h[r]);
                         }
                     }
                 }

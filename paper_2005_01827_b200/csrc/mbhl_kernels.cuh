@@ -196,8 +196,20 @@ __global__ void __launch_bounds__(128) k_sparse_eval(const WalkerConst* __restri
 //   C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows)
 //   D. backward sweep s_r = g_r - c'_r s_{r+1}
 //   E. c_j, d_j of every interval; records written as 128-byte half records
-// coef layout [walker][mode][interval][q][4] = (y_j, s_j, c_j, d_j); phase row: y_j reduced mod 1 cycle.
+// coef layout [walker][mode][interval][q][4] = (y_j, s_j, c_j, d_j).  Phase row (q = 1) as the dense kernel wants it:
+// quarter turns, linear term folded in: 4 [(y_j mod 1) - frac(x_j t_coal)], 4 (s_j - t_coal), 4 c_j, 4 d_j, so that
+// the total phase of a bin is ONE cubic in u = f - x_j (mbhl_sparse converts back to cycles on export).
 // ---------------------------------------------------------------------------------------------
+constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
+
+// frac(f * t) in cycles with the product taken exactly (reading G9): f and t are the supplied doubles.
+__device__ __forceinline__ double linear_cycles(double f, double t) {
+    const double p = f * t;
+    const double e = fma(f, t, -p);
+    const double pr = (p + kRoundMagic) - kRoundMagic;
+    return (p - pr) + e;
+}
+
 __device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
 
 constexpr int kSplineQ = 4;              // quantities per CTA
@@ -232,6 +244,7 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
     const int tid = threadIdx.x;
     double* cout = coef + bm * (int64_t)(S - 1) * kCoefStride + half * (kSplineQ * 4);
     const bool active = wc[b].valid && wc[b].mode[mi].active;
+    const double t_coal = wc[b].t_coal;
     if (!active) {
         for (int idx = tid; idx < (S - 1) * kSplineQ * 2; idx += blockDim.x) {
             const int j = idx >> 3, i = idx & 7;
@@ -357,10 +370,18 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
         const double dl = (y1 - y0) * hinv;
         const double cc = (3.0 * dl - 2.0 * s0 - s1) * hinv;
         const double dd = (s0 + s1 - 2.0 * dl) * (hinv * hinv);
-        if (half == 0 && q == 1) y0 -= rint(y0);
+        double s0w = s0, ccw = cc, ddw = dd;
+        if (half == 0 && q == 1) {
+            // phase row: quarter turns, with the linear term -f t_coal of the total phase (reading G9) folded in.
+            // f t_coal = x_j t_coal + u t_coal: the first product is reduced mod 1 exactly, the second joins the slope.
+            y0 = 4.0 * ((y0 - rint(y0)) - linear_cycles(xk[pad_idx(j)], t_coal));
+            s0w = 4.0 * (s0 - t_coal);
+            ccw = 4.0 * cc;
+            ddw = 4.0 * dd;
+        }
         double2* o = reinterpret_cast<double2*>(cout + (int64_t)j * kCoefStride + q * 4);
-        o[0] = make_double2(y0, s0);
-        o[1] = make_double2(cc, dd);
+        o[0] = make_double2(y0, s0w);
+        o[1] = make_double2(ccw, ddw);
     }
 }
 
@@ -415,7 +436,6 @@ __constant__ double c_sc[13] = {1.5707963267948966, -0.6459640975062443, 0.07969
 #define kC4 c_sc[10]
 #define kC5 c_sc[11]
 #define kC6 c_sc[12]
-constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
 
 // sin and cos of p4 quarter turns (angle = p4 pi/2), any |p4| < 2^51.  No conversions, no divides: the
 // nearest integer comes from the magic-number add, the quadrant from the low word of that sum.
@@ -439,14 +459,6 @@ __device__ __forceinline__ void sincos_qturn(double p4, double& sn, double& cs) 
     cs = __hiloint2double(__double2hiint(b) ^ (((n + 1) & 2) << 30), __double2loint(b));
 }
 
-// frac(f * t) in cycles with the product taken exactly (reading G9): f and t are the supplied doubles.
-__device__ __forceinline__ double linear_cycles(double f, double t) {
-    const double p = f * t;
-    const double e = fma(f, t, -p);
-    const double pr = (p + kRoundMagic) - kRoundMagic;
-    return (p - pr) + e;
-}
-
 // Locates the spline interval of frequency f (ln f = lf) on the log-spaced knots x[0..S-1].
 __device__ __forceinline__ int find_interval(const double* __restrict__ x, int S, double f, double lf, double ln_flo,
                                              double inv_dlog) {
@@ -458,8 +470,8 @@ __device__ __forceinline__ int find_interval(const double* __restrict__ x, int S
 }
 
 // One mode's contribution at one bin from the record `rec` (8 cubics in u = f - f_j): used by the
-// per-bin path of the dense kernel and by mbhl_template.  lin4 = 4 frac(f t_coal); amplitude scaled by `gate`.
-__device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, double u, double lin4, double gate, double h[6]) {
+// per-bin path of the dense kernel and by mbhl_template.  Amplitude scaled by `gate`.
+__device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, double u, double gate, double h[6]) {
     double v[MBHL_NQ];
 #pragma unroll
     for (int q = 0; q < MBHL_NQ; q += 1) {
@@ -468,7 +480,7 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
         v[q] = fma(fma(fma(c23.y, u, c23.x), u, c01.y), u, c01.x);
     }
     double sn, cs;
-    sincos_qturn(fma(v[1], 4.0, -lin4), sn, cs);
+    sincos_qturn(v[1], sn, cs);
     const double amp = v[0] * gate;
     const double are = amp * cs, aim = amp * sn;
     h[0] = fma(are, v[2], fma(-aim, v[3], h[0]));
@@ -530,7 +542,6 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
     if (c.valid) {
         const double f = freqs[k];
         const double lf = log(f);
-        const double lin4 = 4.0 * linear_cycles(f, c.t_coal);
         for (int mi = 0; mi < MBHL_NMODE; ++mi) {
             const ModeConst& mc = c.mode[mi];
             if (!mc.active || !(f >= mc.f_lo) || !(f <= mc.f_hi)) continue;
@@ -538,7 +549,7 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
                 double q[MBHL_NQ];
                 smooth_quantities(c, mi, f, q);
                 double sn, cs;
-                sincos_qturn(fma(q[1] - rint(q[1]), 4.0, -lin4), sn, cs);
+                sincos_qturn(fma(q[1] - rint(q[1]), 4.0, -4.0 * linear_cycles(f, c.t_coal)), sn, cs);
                 const double are = q[0] * cs, aim = q[0] * sn;
                 h[0] += are * q[2] - aim * q[3];
                 h[1] += are * q[3] + aim * q[2];
@@ -550,7 +561,7 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
                 const double* x = knots + (b * MBHL_NMODE + mi) * S;
                 const int j = find_interval(x, S, f, lf, mc.ln_flo, mc.inv_dlog);
                 const double u = f - x[j];
-                mode_contrib(coef + ((b * MBHL_NMODE + mi) * (int64_t)(S - 1) + j) * kCoefStride, u, lin4, 1.0, h);
+                mode_contrib(coef + ((b * MBHL_NMODE + mi) * (int64_t)(S - 1) + j) * kCoefStride, u, 1.0, h);
             }
         }
     }
@@ -568,6 +579,29 @@ __global__ void k_export_y(const double* __restrict__ y, int64_t n_rows, int S, 
     const int64_t row = i / S;
     const double v = y[i];
     out[i] = ((row % MBHL_NQ) == 1) ? v * kTwoPi : v;
+}
+
+// mbhl_sparse: coefficient records with the phase row converted back to the documented form (cycles, y_j in
+// [-1/2, 1/2], no linear term): one thread per (walker, mode, interval, quantity)
+__global__ void k_export_coef(const WalkerConst* __restrict__ wc, const double* __restrict__ knots, const double* __restrict__ coef,
+                              int64_t n_bm, int S, double* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bm * (S - 1) * MBHL_NQ) return;
+    const int q = (int)(i % MBHL_NQ);
+    const int64_t ij = i / MBHL_NQ;
+    const int64_t bm = ij / (S - 1);
+    const int j = (int)(ij - bm * (S - 1));
+    double2 a = reinterpret_cast<const double2*>(coef)[2 * i], c = reinterpret_cast<const double2*>(coef)[2 * i + 1];
+    const WalkerConst& w = wc[bm / MBHL_NMODE];
+    if (q == 1 && w.valid && w.mode[bm % MBHL_NMODE].active) {
+        const double t = w.t_coal;
+        double y = 0.25 * a.x + linear_cycles(knots[bm * S + j], t);
+        y -= rint(y);
+        a = make_double2(y, 0.25 * a.y + t);
+        c = make_double2(0.25 * c.x, 0.25 * c.y);
+    }
+    reinterpret_cast<double2*>(out)[2 * i] = a;
+    reinterpret_cast<double2*>(out)[2 * i + 1] = c;
 }
 
 // FP64 peak probe: 8 independent DFMA chains per thread

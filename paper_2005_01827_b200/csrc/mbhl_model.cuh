@@ -640,8 +640,17 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
             f_lo = fmax(f_top, f_min);
         } else {
             if (x0 < 0.0) {
+                // the time to coalescence tau = t_coal - t_22 falls off like x^(-8/3) (P6), so tau^(-3/8) is nearly
+                // linear in x: the secant steps run on g(x) = tau(x)^(-3/8) - t_coal^(-3/8), which has the sign of t_22
                 const double xa = mc.aP[0] * (f_min * c.M_s);        // t22(xa) = t_min < 0 <= t_top
-                x0 = bracketed_root(t22, xa, t_min, kFPhiIns, t_top, 4e-16 * fabs(c.t_coal) + 1e-12);
+                const double g0 = pow(c.t_coal, -0.375);
+                auto g = [&](double x22) {
+                    const double tau = c.t_coal - t22(x22);
+                    return (tau > 0.0) ? pow(tau, -0.375) - g0 : 1e300;
+                };
+                const double ga = pow(c.t_coal - t_min, -0.375) - g0;
+                const double gb = (c.t_coal - t_top > 0.0) ? pow(c.t_coal - t_top, -0.375) - g0 : 1e300;
+                x0 = bracketed_root(g, xa, ga, kFPhiIns, gb, 4e-16 * g0);
             }
             f_lo = fmax(f_min, x0 * (0.5 * m) / c.M_s);
         }
