@@ -448,7 +448,7 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": "k_dense", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                     "frac": achieved / fp64_peak,
+                     "frac": achieved / fp64_peak, "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
                      # dram__bytes_read.sum + dram__bytes_write.sum of one k_dense launch, from the committed ncu --set full capture
                      "traffic": 2.04e9 if args.config == 2 else None, "traffic_source": "profiles/r01_dense_c2_final_ncu.txt (bytes per launch)",
                      "peak_source": "DFMA-chain probe measured in this run (nominal 148 SM x 64 lanes x 2 x 1.965 GHz = %.1f)" % NOMINAL_FP64_TFLOPS,

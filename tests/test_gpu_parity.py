@@ -296,3 +296,21 @@ def test_loglike_parity_config2_full_size_in_the_bench_launch_configuration(tabl
         assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (b, ll[b], rll)
         assert abs(hh[b] - rhh) <= 1e-8 * rhh, (b, hh[b], rhh)
     M.mbhl_free(ctx)
+
+
+def test_batches_beyond_the_grid_limit_are_sliced(table, cfg0):
+    # B > 65535 walkers: the library processes slices of 32768; every copy of a walker must give the same number
+    n = 3 * 512 + 5
+    sl = slice(30000, 30000 + n)
+    ctx = M.mbhl_init(dev(cfg0["freqs"][sl]), dev(cfg0["data"][:, sl]), dev(cfg0["psd"][:, sl]), sparse_points=32)
+    base = cfg0["params"][:4]
+    ref = M.mbhl_loglike(ctx, dev(base)).cpu().numpy()
+    B = 70003
+    big = np.tile(base, (B // 4 + 1, 1))[:B]
+    dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(big))]
+    assert ll.shape == (B,)
+    # slices of 32768 walkers and the last partial slice take other launch shapes: same sums up to rounding order
+    dd = M.mbhl_data_norm(ctx)
+    for k in range(4):
+        assert np.max(np.abs(ll[k::4] - ref[k])) <= 1e-12 * (dd + np.max(hh[k::4]))
+    M.mbhl_free(ctx)
