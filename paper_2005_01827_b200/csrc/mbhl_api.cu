@@ -67,6 +67,8 @@ DensePlan dense_plan(int64_t B, int n_chunks) {
     return p;
 }
 
+constexpr int64_t kSliceBatch = 32768;   // walkers per pass of the hot path; larger batches are processed in slices
+
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 int n_chunks_of(int64_t N) { return (int)((N + kChunk - 1) / kChunk); }
@@ -363,10 +365,10 @@ int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d
     if (!ctx) return MBHL_EINVAL;
     if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
     if (B == 0) return MBHL_OK;
-    if (B > 65535) {
-        // grid.y limit of the dense kernel: process in slices
-        for (int64_t o = 0; o < B; o += 32768) {
-            const int64_t n = (B - o < 32768) ? (B - o) : 32768;
+    if (B > kSliceBatch) {
+        // large batches go in slices, so the workspace stays that of one slice
+        for (int64_t o = 0; o < B; o += kSliceBatch) {
+            const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
             int rc = mbhl_loglike_parts(ctx, params + o * MBHL_NPARAM, n, d_h ? d_h + o : nullptr, h_h ? h_h + o : nullptr,
                                         logL ? logL + o : nullptr);
             if (rc != MBHL_OK) return rc;
@@ -394,6 +396,13 @@ int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, doubl
     if (!ctx) return MBHL_EINVAL;
     if (B < 0 || (B > 0 && (!params_host || !logL_host))) return fail(ctx, MBHL_EINVAL, "bad host buffers");
     if (B == 0) return MBHL_OK;
+    if (B > kSliceBatch) {   // the staging areas live in the workspace of ONE slice: go slice by slice
+        for (int64_t o = 0; o < B; o += kSliceBatch) {
+            const int rc = mbhl_loglike_host(ctx, params_host + o * MBHL_NPARAM, (B - o < kSliceBatch) ? (B - o) : kSliceBatch, logL_host + o);
+            if (rc != MBHL_OK) return rc;
+        }
+        return MBHL_OK;
+    }
     CU(cudaSetDevice(ctx->device));
     char* base;
     int rc = get_workspace(ctx, B, &base);
@@ -432,6 +441,13 @@ int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* 
     if (!ctx) return MBHL_EINVAL;
     if (B < 0 || (B > 0 && (!theta || !logL))) return fail(ctx, MBHL_EINVAL, "bad theta/logL/B");
     if (B == 0) return MBHL_OK;
+    if (B > kSliceBatch) {
+        for (int64_t o = 0; o < B; o += kSliceBatch) {
+            const int rc = mbhl_loglike_sampled(ctx, theta + o * MBHL_NPARAM, (B - o < kSliceBatch) ? (B - o) : kSliceBatch, logL + o);
+            if (rc != MBHL_OK) return rc;
+        }
+        return MBHL_OK;
+    }
     CU(cudaSetDevice(ctx->device));
     char* base;
     int rc = get_workspace(ctx, B, &base);

@@ -313,4 +313,8 @@ def test_batches_beyond_the_grid_limit_are_sliced(table, cfg0):
     dd = M.mbhl_data_norm(ctx)
     for k in range(4):
         assert np.max(np.abs(ll[k::4] - ref[k])) <= 1e-12 * (dd + np.max(hh[k::4]))
+    # the host-buffer entry point stages parameters in the workspace: sliced the same way
+    lh = torch.empty(B, dtype=torch.float64).pin_memory()
+    M.mbhl_loglike_host(ctx, torch.from_numpy(big.copy()).pin_memory(), lh)
+    assert np.array_equal(lh.numpy(), ll)
     M.mbhl_free(ctx)

@@ -75,6 +75,12 @@ def test_loglike_sampled_parity(table, small):
     bad[3, 10] = np.nan
     out = M.mbhl_loglike_sampled(ctx, dev(bad)).cpu().numpy()
     assert np.all(np.isneginf(out))
+    # a batch larger than one slice of the hot path (32768 walkers)
+    n = 40001
+    big = np.tile(th, (n // th.shape[0] + 1, 1))[:n]
+    out = M.mbhl_loglike_sampled(ctx, dev(big)).cpu().numpy()
+    for b in range(th.shape[0]):
+        assert np.max(np.abs(out[b::th.shape[0]] - ll[b])) <= 1e-9 * (1.0 + abs(ll[b]))
     M.mbhl_free(ctx)
 
 
