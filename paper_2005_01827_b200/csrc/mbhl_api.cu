@@ -149,7 +149,7 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     const bool tm = ctx->timing && with_coef;
     if (tm) ctx->ev = ctx->evs[ctx->n_timed % mbhl_ctx::kSlots];
     if (tm) cudaEventRecord(ctx->ev[0], ctx->stream);
-    k_walker_consts<<<(unsigned)((B + 63) / 64), 64, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
+    k_walker_consts<<<(unsigned)((B + kConstsWarps - 1) / kConstsWarps), 32 * kConstsWarps, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
                                                                       ctx->mode_mask, ctx->freqs, (int)ctx->N, ctx->df, wc,
                                                                       (DenseWalker*)(base + L.dense));
     if (tm) cudaEventRecord(ctx->ev[1], ctx->stream);

@@ -109,22 +109,22 @@ __device__ inline int last_bin_le(const double* __restrict__ f, int N, double f0
     return k - 1;
 }
 
-__global__ void __launch_bounds__(64) k_walker_consts(const double* __restrict__ params, int64_t B, double t0, double f_min,
+constexpr int kConstsWarps = 4;      // walkers per CTA of k_walker_consts (one warp each)
+
+__global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const double* __restrict__ params, int64_t B, double t0, double f_min,
                                                       double f_max, int S, uint32_t mode_mask, const double* __restrict__ freqs,
                                                       int N, double df, WalkerConst* __restrict__ out,
                                                       DenseWalker* __restrict__ dw) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ WalkerConst s_c[kConstsWarps];
+    __shared__ DenseWalker s_d[kConstsWarps];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t b = (int64_t)blockIdx.x * kConstsWarps + warp;
     if (b >= B) return;
-    WalkerConst c;
-    build_walker(params + b * 11, t0, f_min, f_max, S, mode_mask, c);
-    out[b] = c;
-    DenseWalker d;
-    d.t_coal = c.valid ? c.t_coal : 0.0;
-    d.valid = c.valid;
-    d.pad_ = 0;
-    long long pairs = 0;
-    int lo[MBHL_NMODE], hi[MBHL_NMODE];
-    for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+    WalkerConst& c = s_c[warp];
+    DenseWalker& d = s_d[warp];
+    const int mi = lane % MBHL_NMODE;                  // lanes 6.. repeat the work of lanes 0-5 (identical stores)
+    build_walker(params + b * 11, t0, f_min, f_max, S, mode_mask, c, mi, mi + 1);
+    {
         DenseMode m;
         m.k_lo = 1; m.k_hi = 0; m.ln_flo = 0.0; m.inv_dlog = 0.0;
         if (c.valid && c.mode[mi].active) {
@@ -132,28 +132,41 @@ __global__ void __launch_bounds__(64) k_walker_consts(const double* __restrict__
             m.k_hi = last_bin_le(freqs, N, f_min, 1.0 / df, c.mode[mi].f_hi);
             m.ln_flo = c.mode[mi].ln_flo;
             m.inv_dlog = c.mode[mi].inv_dlog;
-            if (m.k_hi >= m.k_lo) pairs += (long long)(m.k_hi - m.k_lo + 1);
-            else { m.k_lo = 1; m.k_hi = 0; }
+            if (m.k_hi < m.k_lo) { m.k_lo = 1; m.k_hi = 0; }
         }
-        lo[mi] = m.k_lo; hi[mi] = m.k_hi;
         d.mode[mi] = m;
     }
-    // bins covered by at least one mode: length of the union of the six ranges
-    long long bins = 0;
-    int done_to = -1;                               // everything <= done_to is already counted
-    for (int it = 0; it < MBHL_NMODE; ++it) {
-        int best = -1;
-        for (int mi = 0; mi < MBHL_NMODE; ++mi)
-            if (hi[mi] >= lo[mi] && hi[mi] > done_to && (best < 0 || lo[mi] < lo[best])) best = mi;
-        if (best < 0) break;
-        const int a = max(lo[best], done_to + 1);
-        bins += (long long)(hi[best] - a + 1);
-        done_to = hi[best];
-        // ranges fully below done_to are skipped by the hi > done_to test above
+    __syncwarp();
+    if (lane == 0) {
+        d.t_coal = c.valid ? c.t_coal : 0.0;
+        d.valid = c.valid;
+        d.pad_ = 0;
+        long long pairs = 0;
+        int lo[MBHL_NMODE], hi[MBHL_NMODE];
+        for (int k = 0; k < MBHL_NMODE; ++k) {
+            lo[k] = d.mode[k].k_lo; hi[k] = d.mode[k].k_hi;
+            if (hi[k] >= lo[k]) pairs += (long long)(hi[k] - lo[k] + 1);
+        }
+        // bins covered by at least one mode: length of the union of the six ranges
+        long long bins = 0;
+        int done_to = -1;                               // everything <= done_to is already counted
+        for (int it = 0; it < MBHL_NMODE; ++it) {
+            int best = -1;
+            for (int k = 0; k < MBHL_NMODE; ++k)
+                if (hi[k] >= lo[k] && hi[k] > done_to && (best < 0 || lo[k] < lo[best])) best = k;
+            if (best < 0) break;
+            const int a = max(lo[best], done_to + 1);
+            bins += (long long)(hi[best] - a + 1);
+            done_to = hi[best];
+        }
+        d.pairs = pairs;
+        d.bins = bins;
     }
-    d.pairs = pairs;
-    d.bins = bins;
-    dw[b] = d;
+    __syncwarp();
+    // coalesced copies of the two records to global memory
+    static_assert(sizeof(WalkerConst) % 8 == 0 && sizeof(DenseWalker) % 8 == 0, "records are copied as doubles");
+    for (int i = lane; i < (int)(sizeof(WalkerConst) / 8); i += 32) reinterpret_cast<double*>(out + b)[i] = reinterpret_cast<const double*>(&c)[i];
+    for (int i = lane; i < (int)(sizeof(DenseWalker) / 8); i += 32) reinterpret_cast<double*>(dw + b)[i] = reinterpret_cast<const double*>(&d)[i];
 }
 
 // ---------------------------------------------------------------------------------------------

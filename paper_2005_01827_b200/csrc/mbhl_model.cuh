@@ -371,8 +371,11 @@ __device__ inline double bracketed_root(F fn, double a, double fa, double b, dou
     return b;
 }
 
+// Everything per walker.  The per-mode parts run for the modes mode_lo <= mi < mode_hi only: k_walker_consts gives a warp
+// to every walker, all lanes run the common part redundantly on one shared-memory record (identical stores)
+// and lane L fills mode L % 6.
 __device__ inline void build_walker(const double* __restrict__ p, double t0, double f_min, double f_max, int S,
-                                    uint32_t mode_mask, WalkerConst& c) {
+                                    uint32_t mode_mask, WalkerConst& c, int mode_lo, int mode_hi) {
     const double M_T = p[0], q_in = p[1], a1 = p[2], a2 = p[3], D_L = p[4];
     const double phi_ref = p[5], inc = p[6], lam = p[7], beta = p[8], psi_pol = p[9], t_ref = p[10];
     bool ok = true;
@@ -381,6 +384,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     c.valid = ok ? 1 : 0;
     c.pad_ = 0;
     for (int mi = 0; mi < MBHL_NMODE; ++mi) c.mode[mi].active = 0;
+    __syncwarp();                                       // every lane is past the reset before a lane fills its mode
     if (!ok) return;
 
     const double q = (q_in >= 1.0) ? q_in : 1.0 / q_in;
@@ -420,7 +424,8 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     {
         const double oma = 1.0 - af;
         const double inv = 1.0 / (kTwoPi * (1.0 - Erad));
-        for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+        for (int mi = 0; mi < mode_hi; ++mi) {
+            if (mi != 0 && mi < mode_lo) continue;           // mode (2,2) is needed by everyone
             const double* t6 = T + MT_qnm_22_f1 + 6 * mi;
             const double om = t6[0] + t6[1] * pow(oma, t6[2]);
             const double Q = t6[3] + t6[4] * pow(oma, t6[5]);
@@ -567,7 +572,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     psi22(c, f_i22P, &psi_i, &dtmp);
     psi22(c, c.fRD, &psi_r, &dtmp);
     const double ampbase = kPi * sqrt(2.0 * eta / 3.0);
-    for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+    for (int mi = mode_lo; mi < mode_hi; ++mi) {
         ModeConst& mc = c.mode[mi];
         const int l = c_mode_l[mi], m = c_mode_m[mi];
         mc.fiA = 0.5 * m * f_i22A;
@@ -626,7 +631,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     };
     const double t_top = t22(kFPhiIns);                 // t_lm at the end of every mode's inspiral branch
     double x0 = -1.0;
-    for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+    for (int mi = mode_lo; mi < mode_hi; ++mi) {
         if (!((mode_mask >> mi) & 1u)) continue;
         ModeConst& mc = c.mode[mi];
         const int m = c_mode_m[mi];
