@@ -318,3 +318,17 @@ def test_batches_beyond_the_grid_limit_are_sliced(table, cfg0):
     M.mbhl_loglike_host(ctx, torch.from_numpy(big.copy()).pin_memory(), lh)
     assert np.array_equal(lh.numpy(), ll)
     M.mbhl_free(ctx)
+
+
+def test_tiny_grids_and_few_knots(table, cfg0):
+    # the smallest inputs the boundary accepts (N >= 4 bins, S >= 8 knots) and a handful of sizes around the tile edges
+    for n, S, k0 in ((4, 8, 20000), (7, 8, 100), (127, 9, 40000), (129, 17, 60000), (513, 33, 5)):
+        sl = slice(k0, k0 + n)
+        f, d, s_ = cfg0["freqs"][sl].copy(), np.ascontiguousarray(cfg0["data"][:, sl]), np.ascontiguousarray(cfg0["psd"][:, sl])
+        ctx = M.mbhl_init(dev(f), dev(d), dev(s_), sparse_points=S)
+        p = cfg0["params"][:3]
+        ll = M.mbhl_loglike(ctx, dev(p)).cpu().numpy()
+        for b in range(3):
+            ref = L.loglike_parts(table, p[b], f, d, s_, S, 0.0)[2]
+            assert abs(ll[b] - ref) <= 1e-6 * (1.0 + abs(ref)), (n, S, b, ll[b], ref)
+        M.mbhl_free(ctx)
