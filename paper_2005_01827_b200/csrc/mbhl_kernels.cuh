@@ -179,8 +179,13 @@ __global__ void __launch_bounds__(128) k_sparse_eval(const WalkerConst* __restri
     const int64_t b = bm / MBHL_NMODE;
     const int mi = (int)(bm - b * MBHL_NMODE);
     const int s = blockIdx.y * blockDim.x + threadIdx.x;
+    // the CTA's 128 knots belong to one (walker, mode): its constants are read from shared memory
+    __shared__ WalkerConst s_c;
+    for (int i = threadIdx.x; i < (int)(sizeof(WalkerConst) / 8); i += blockDim.x)
+        reinterpret_cast<double*>(&s_c)[i] = reinterpret_cast<const double*>(wc + b)[i];
+    __syncthreads();
     if (s >= S) return;
-    const WalkerConst& c = wc[b];
+    const WalkerConst& c = s_c;
     double q[MBHL_NQ];
     double f = 0.0;
     if (c.valid && c.mode[mi].active) {
