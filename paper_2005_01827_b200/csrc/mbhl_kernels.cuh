@@ -234,9 +234,13 @@ constexpr int kSplineQ = 4;              // quantities per CTA
 constexpr int kSplineHaloPivot = 16;
 constexpr int kSplineHaloSweep = 32;
 
+// Row strides (in doubles) congruent to 4 mod 16: the last phase reads rows q = 0..3 at intervals j..j+3 from one
+// half-warp, and 4 q + j then covers the 16 bank pairs once (a stride of S or S + S/32 + 1 gives 4-way conflicts).
+__host__ __device__ inline int spline_stride(int n) { return n + ((4 - n % 16) + 16) % 16; }
+__host__ __device__ inline int spline_sp(int S) { return spline_stride(S + (S >> 5) + 1); }
+
 __host__ __device__ inline size_t spline_smem_bytes(int S) {
-    const int SP = S + (S >> 5) + 1;
-    return (size_t)(5 + kSplineQ) * SP * sizeof(double) + (size_t)kSplineQ * S * sizeof(double);
+    return (size_t)(5 + kSplineQ) * spline_sp(S) * sizeof(double) + (size_t)kSplineQ * spline_stride(S) * sizeof(double);
 }
 
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
@@ -247,14 +251,14 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) 
 __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ wc, int S, const double* __restrict__ knots,
                                                 const double* __restrict__ y, double* __restrict__ coef) {
     extern __shared__ double sm[];
-    const int SP = S + (S >> 5) + 1;
+    const int SP = spline_sp(S), SY = spline_stride(S);
     double* xk = sm;                     // knots                                  [SP]
     double* ih = xk + SP;                // 1 / h_r, h_r = x_{r+1} - x_r          [SP]
     double* cps = ih + SP;               // pivots c'_r                            [SP]
     double* ivs = cps + SP;              // 1 / (d_r - a_r c'_{r-1})               [SP]
     double* mls = ivs + SP;              // a_r / (d_r - a_r c'_{r-1})             [SP]
     double* A1 = mls + SP;               // b, then g, then the slopes s (in place) [4][SP]
-    double* Y = A1 + kSplineQ * SP;      // y values of the 4 quantities           [4][S], unpadded
+    double* Y = A1 + kSplineQ * SP;      // y values of the 4 quantities           [4][SY]
     const int64_t bm = blockIdx.x >> 1;
     const int half = blockIdx.x & 1;
     const int64_t b = bm / MBHL_NMODE;
@@ -275,7 +279,7 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
     const double* yg = y + (bm * MBHL_NQ + half * kSplineQ) * S;
     for (int i = tid; i < S; i += blockDim.x) cp_async8(xk + pad_idx(i), xg + i);
     asm volatile("cp.async.commit_group;" ::: "memory");
-    for (int i = tid; i < kSplineQ * S; i += blockDim.x) cp_async8(Y + i, yg + i);
+    for (int i = tid; i < kSplineQ * S; i += blockDim.x) cp_async8(Y + (i / S) * SY + i % S, yg + i);
     asm volatile("cp.async.commit_group;" ::: "memory");
     asm volatile("cp.async.wait_group 1;" ::: "memory");
     __syncthreads();
@@ -313,7 +317,7 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
     // B. scaled right-hand sides of the slope system, all rows in parallel
     for (int idx = tid; idx < kSplineQ * S; idx += blockDim.x) {
         const int q = idx / S, r = idx - q * S;
-        const double* yq = Y + q * S;
+        const double* yq = Y + q * SY;
         double v;
         if (r == 0) {
             const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
@@ -382,8 +386,8 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
     for (int idx = tid; idx < (S - 1) * kSplineQ; idx += blockDim.x) {
         const int j = idx >> 2, q = idx & 3;
         const double hinv = ih[pad_idx(j)];
-        double y0 = Y[q * S + j];
-        const double y1 = Y[q * S + j + 1];
+        double y0 = Y[q * SY + j];
+        const double y1 = Y[q * SY + j + 1];
         const double s0 = A1[q * SP + pad_idx(j)], s1 = A1[q * SP + pad_idx(j + 1)];
         const double dl = (y1 - y0) * hinv;
         const double cc = (3.0 * dl - 2.0 * s0 - s1) * hinv;
