@@ -158,7 +158,7 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     ctx->launches += 2;
     if (tm) cudaEventRecord(ctx->ev[2], ctx->stream);
     if (with_coef) {
-        k_spline<<<(unsigned)(B * MBHL_NMODE * 2), 128, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
+        k_spline<<<(unsigned)(B * MBHL_NMODE * 2), kSplineThreads, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
         ctx->launches += 1;
     }
     CU(cudaGetLastError());

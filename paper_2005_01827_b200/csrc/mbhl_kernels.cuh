@@ -231,6 +231,7 @@ __device__ __forceinline__ double linear_cycles(double f, double t) {
 __device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
 
 constexpr int kSplineQ = 4;              // quantities per CTA
+constexpr int kSplineThreads = 256;      // 8 warps for the row-parallel phases; warps 0-3 run the sweeps (one quantity each)
 constexpr int kSplineHaloPivot = 16;
 constexpr int kSplineHaloSweep = 32;
 
@@ -248,7 +249,7 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) 
                  : "memory");
 }
 
-__global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ wc, int S, const double* __restrict__ knots,
+__global__ void __launch_bounds__(kSplineThreads) k_spline(const WalkerConst* __restrict__ wc, int S, const double* __restrict__ knots,
                                                 const double* __restrict__ y, double* __restrict__ coef) {
     extern __shared__ double sm[];
     const int SP = spline_sp(S), SY = spline_stride(S);
@@ -337,7 +338,7 @@ __global__ void __launch_bounds__(128) k_spline(const WalkerConst* __restrict__ 
     __syncthreads();
     // C, D. sweeps in place: warp = quantity, lane = block of rows.  A lane first copies the halo rows it needs
     // from its neighbour's block into registers, so the neighbour may overwrite them afterwards.
-    {
+    if (tid < 32 * kSplineQ) {
         const int q = tid >> 5, lane = tid & 31;
         const int m = (S + 31) / 32;
         const int own0 = lane * m, own1 = min(S, own0 + m);
