@@ -150,7 +150,10 @@ struct PairDesc {
 };
 
 constexpr int kRecSlots = 2 * kPairs;                                                       // two records per pair
-constexpr int kDenseSmemBytes = kTileBytes + kRecSlots * kCoefStride * (int)sizeof(double);   // 40 KB tile + 24 KB records
+// per-warp scratch of the general path: the records and knots of up to kGenSlots consecutive intervals
+constexpr int kGenSlots = 6;
+constexpr int kGenDoubles = kGenSlots * kCoefStride + 8;
+constexpr int kDenseSmemBytes = (kTileDoubles + kRecSlots * kCoefStride + (kDenseThreads / 32) * kGenDoubles) * (int)sizeof(double);   // 40 KB tile + 24 KB records + 6.2 KB scratch
 
 __device__ __forceinline__ void stage_record(double* dst, const double* __restrict__ src) {
 #pragma unroll
@@ -163,6 +166,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
     extern __shared__ __align__(128) double s_dyn[];
     double* const s_tile = s_dyn;                                   // [10][512] staged data tile
     double* const s_rec = s_dyn + kTileDoubles;                     // [kRecSlots][32] staged coefficient records
+    double* const s_gen = s_rec + kRecSlots * kCoefStride + (threadIdx.x >> 5) * kGenDoubles;   // this warp's general-path scratch
     __shared__ DenseWalker s_dw[kMaxW];
     __shared__ double s_xj[kRecSlots];                              // knot x_j of each staged record
     __shared__ PairDesc s_desc[kPairs];
@@ -350,6 +354,26 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                     const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
                     if (ja_m == jb_m && full_m) {
                         mode_uniform<false>(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, f, h);
+                    } else if (jb_m - ja_m < kGenSlots) {
+                        // a few intervals in the warp tile: their records and knots are copied to this warp's scratch with
+                        // independent loads (one L2 round trip), then every bin looks its interval up in shared memory
+                        const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
+                        const int nrec = jb_m - ja_m + 1;
+                        __syncwarp();
+                        for (int i = lane; i < nrec * (kCoefStride / 2); i += 32)
+                            reinterpret_cast<double2*>(s_gen)[i] = __ldg(reinterpret_cast<const double2*>(cbase + (int64_t)ja_m * kCoefStride) + i);
+                        double* const gx = s_gen + kGenSlots * kCoefStride;
+                        if (lane <= nrec) gx[lane] = __ldg(x + ja_m + lane);
+                        __syncwarp();
+#pragma unroll
+                        for (int r = 0; r < kDenseR; ++r) {
+                            const int k = kt0 + lane + 32 * r;
+                            if (k < k_lo || k > k_hi) continue;
+                            int j = ((nrec - 1) * (lane + 32 * r)) / kWarpTile;
+                            while (j > 0 && f[r] < gx[j]) --j;
+                            while (j < nrec - 1 && f[r] >= gx[j + 1]) ++j;
+                            mode_contrib<false>(s_gen + j * kCoefStride, f[r] - gx[j], 1.0, h[r]);
+                        }
                     } else {
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
 #pragma unroll

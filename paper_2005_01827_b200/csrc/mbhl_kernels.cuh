@@ -494,12 +494,14 @@ __device__ __forceinline__ int find_interval(const double* __restrict__ x, int S
 
 // One mode's contribution at one bin from the record `rec` (8 cubics in u = f - f_j): used by the
 // per-bin path of the dense kernel and by mbhl_template.  Amplitude scaled by `gate`.
+// kGlobal: the record sits in global memory (read-only path); otherwise in shared memory.
+template <bool kGlobal = true>
 __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, double u, double gate, double h[6]) {
     double v[MBHL_NQ];
 #pragma unroll
     for (int q = 0; q < MBHL_NQ; q += 1) {
-        const double2 c01 = __ldg(reinterpret_cast<const double2*>(rec + q * 4));
-        const double2 c23 = __ldg(reinterpret_cast<const double2*>(rec + q * 4 + 2));
+        const double2 c01 = kGlobal ? __ldg(reinterpret_cast<const double2*>(rec + q * 4)) : *reinterpret_cast<const double2*>(rec + q * 4);
+        const double2 c23 = kGlobal ? __ldg(reinterpret_cast<const double2*>(rec + q * 4 + 2)) : *reinterpret_cast<const double2*>(rec + q * 4 + 2);
         v[q] = fma(fma(fma(c23.y, u, c23.x), u, c01.y), u, c01.x);
     }
     double sn, cs;
