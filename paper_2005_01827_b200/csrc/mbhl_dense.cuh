@@ -142,6 +142,50 @@ __device__ __forceinline__ void mode_uniform(const double* __restrict__ rec, dou
     }
 }
 
+// One mode's contribution when the kDenseR bins of a lane lie in different spline intervals whose records sit in
+// shared memory: bin r reads its own record rec[r] at u[r] = f - x_j, amplitude gated by gate[r] (0 for bins out of
+// band, whose rec[r] is any valid record).  Same lockstep arithmetic as mode_uniform.
+__device__ __forceinline__ void mode_perbin(const double* const (&rec)[kDenseR], const double (&u)[kDenseR],
+                                            const double (&gate)[kDenseR], double (&h)[kDenseR][6]) {
+    double are[kDenseR], aim[kDenseR];
+    {
+        double p4[kDenseR], sn[kDenseR], cs[kDenseR], amp[kDenseR];
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) {
+            const double2 p01 = *reinterpret_cast<const double2*>(rec[r] + 4);
+            const double2 p23 = *reinterpret_cast<const double2*>(rec[r] + 6);
+            p4[r] = fma(fma(fma(p23.y, u[r], p23.x), u[r], p01.y), u[r], p01.x);
+        }
+        sincos_qturn_x(p4, sn, cs);
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) {
+            const double2 a01 = *reinterpret_cast<const double2*>(rec[r]);
+            const double2 a23 = *reinterpret_cast<const double2*>(rec[r] + 2);
+            amp[r] = fma(fma(fma(a23.y, u[r], a23.x), u[r], a01.y), u[r], a01.x) * gate[r];
+        }
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) { are[r] = amp[r] * cs[r]; aim[r] = amp[r] * sn[r]; }
+    }
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+        double tre[kDenseR], tim[kDenseR];
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) {
+            const double2 r01 = *reinterpret_cast<const double2*>(rec[r] + 8 + 8 * ch);
+            const double2 r23 = *reinterpret_cast<const double2*>(rec[r] + 10 + 8 * ch);
+            const double2 i01 = *reinterpret_cast<const double2*>(rec[r] + 12 + 8 * ch);
+            const double2 i23 = *reinterpret_cast<const double2*>(rec[r] + 14 + 8 * ch);
+            tre[r] = fma(fma(fma(r23.y, u[r], r23.x), u[r], r01.y), u[r], r01.x);
+            tim[r] = fma(fma(fma(i23.y, u[r], i23.x), u[r], i01.y), u[r], i01.x);
+        }
+#pragma unroll
+        for (int r = 0; r < kDenseR; ++r) {
+            h[r][2 * ch] = fma(are[r], tre[r], fma(-aim[r], tim[r], h[r][2 * ch]));
+            h[r][2 * ch + 1] = fma(are[r], tim[r], fma(aim[r], tre[r], h[r][2 * ch + 1]));
+        }
+    }
+}
+
 // What the prepare step found for one (walker, mode) pair in the current chunk; offsets are bins within the chunk.
 struct PairDesc {
     short a, b;      // in-band bins [a, b]
@@ -365,15 +409,19 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                         double* const gx = s_gen + kGenSlots * kCoefStride;
                         if (lane <= nrec) gx[lane] = __ldg(x + ja_m + lane);
                         __syncwarp();
+                        const double* rec[kDenseR];
+                        double u[kDenseR], gate[kDenseR];
 #pragma unroll
                         for (int r = 0; r < kDenseR; ++r) {
                             const int k = kt0 + lane + 32 * r;
-                            if (k < k_lo || k > k_hi) continue;
                             int j = ((nrec - 1) * (lane + 32 * r)) / kWarpTile;
                             while (j > 0 && f[r] < gx[j]) --j;
                             while (j < nrec - 1 && f[r] >= gx[j + 1]) ++j;
-                            mode_contrib<false>(s_gen + j * kCoefStride, f[r] - gx[j], 1.0, h[r]);
+                            rec[r] = s_gen + j * kCoefStride;
+                            u[r] = f[r] - gx[j];
+                            gate[r] = (k >= k_lo && k <= k_hi) ? 1.0 : 0.0;
                         }
+                        mode_perbin(rec, u, gate, h);
                     } else {
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
 #pragma unroll
