@@ -355,23 +355,36 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                 mode_uniform<false>(s_rec + slot * kCoefStride, s_xj[slot], f, f, h);
             }
             while (m_part) {
-                // band edge or knot inside the warp tile: each staged segment is evaluated on all bins and gated
-                const int mi = __ffs(m_part) - 1;
+                                const int mi = __ffs(m_part) - 1;
                 m_part &= m_part - 1;
                 const int lo0 = __shfl_sync(0xffffffffu, loA, mi), hi0 = __shfl_sync(0xffffffffu, hiA, mi);
                 const int lo1 = __shfl_sync(0xffffffffu, loB, mi), hi1 = __shfl_sync(0xffffffffu, hiB, mi);
-#pragma unroll 1
-                for (int seg = 0; seg < 2; ++seg) {
+                const int slot0 = 2 * (wi * MBHL_NMODE + mi);
+                if (lo0 <= hi0 && lo1 <= hi1) {
+                    // a knot inside the warp tile: every bin reads the staged record of its own side, one pass
+                    const double* rec[kDenseR];
+                    double u[kDenseR], gate[kDenseR];
+                    const double xa = s_xj[slot0], xb = s_xj[slot0 + 1];
+#pragma unroll
+                    for (int r = 0; r < kDenseR; ++r) {
+                        const int o = t0 + lane + 32 * r;
+                        const bool inB = o >= lo1;
+                        rec[r] = s_rec + (slot0 + (inB ? 1 : 0)) * kCoefStride;
+                        u[r] = f[r] - (inB ? xb : xa);
+                        gate[r] = (o >= lo0 && o <= hi1) ? 1.0 : 0.0;
+                    }
+                    mode_perbin(rec, u, gate, h);
+                } else {
+                    // band edge: the one staged segment is evaluated on all bins with the amplitude gated
+                    const int seg = (lo1 <= hi1) ? 1 : 0;
                     const int lo = seg ? lo1 : lo0, hi = seg ? hi1 : hi0;
-                    if (lo > hi) continue;
                     double gate[kDenseR];
 #pragma unroll
                     for (int r = 0; r < kDenseR; ++r) {
                         const int o = t0 + lane + 32 * r;
                         gate[r] = (o >= lo && o <= hi) ? 1.0 : 0.0;
                     }
-                    const int slot = 2 * (wi * MBHL_NMODE + mi) + seg;
-                    mode_uniform<true>(s_rec + slot * kCoefStride, s_xj[slot], f, gate, h);
+                    mode_uniform<true>(s_rec + (slot0 + seg) * kCoefStride, s_xj[slot0 + seg], f, gate, h);
                 }
             }
             if (m_gen) {
