@@ -17,9 +17,10 @@
 //   3. every warp loops over the walkers.  A warp owns 128 consecutive bins, a lane 4 of them (stride 32) and
 //      advances the 4 bins in lockstep (4 independent dependency chains: DFMA latency is 8.4 cycles at an
 //      issue rate of one warp-DFMA per 2 cycles per SM sub-partition, measured).  Fast modes read the staged
-//      record with warp-uniform 16-byte shared-memory loads; the rest (chunks that straddle a knot, band
-//      edges, the lowest ~1e5 bins where intervals are narrower than a chunk) go through the general path:
-//      per-warp interval check with warp-uniform global loads, else a per-bin lookup;
+//      record with warp-uniform 16-byte shared-memory loads; a knot inside the warp tile is one pass in which
+//      every bin reads the staged record of its side; a band edge is one gated pass; chunks with three or more
+//      intervals (the lowest ~1e5 bins) go through the general path: the records and knots of up to 6
+//      consecutive intervals of the warp tile are copied to a per-warp scratch, then looked up per bin;
 //   4. per (walker, bin): <d|h> and <h|h> terms, warp shuffle tree, one shared-memory slot per (warp, walker).
 // One partial per (walker, CTA) leaves the kernel; k_final_reduce adds them in fixed order (bitwise
 // reproducible, no atomics on values).
