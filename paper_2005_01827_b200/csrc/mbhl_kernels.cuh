@@ -409,19 +409,10 @@ __global__ void __launch_bounds__(kSplineThreads) k_spline(const WalkerConst* __
 }
 
 // ---------------------------------------------------------------------------------------------
-// a6 + a7: fused dense kernel.  Interpolates every active mode onto the Fourier bins, sums the modes per
-// bin and accumulates <d|h> and <h|h> (eqs. 2, 3, 11); the template is never written to
-// memory.
-//
-// Work decomposition: a CTA owns a tile of W consecutive walkers and a group of G consecutive 512-bin
-// chunks.  For every chunk the 40 KB data tile (f, w, w d) is staged in shared memory by ONE bulk
-// asynchronous copy (TMA, cp.async.bulk + mbarrier) and reused by all W walkers, so HBM sees each data
-// tile once per walker tile instead of once per walker.  A warp owns 128 consecutive bins (lane + 32 r,
-// r < 4).  Per (walker, mode) the warp checks whether its 128 bins lie in one spline interval (the common
-// case above ~1 mHz): then the 256-byte coefficient record is read with warp-uniform 16-byte loads and
-// shared by the 4 bins of every lane; otherwise every bin looks up its own interval.  The loop body is
-// FP64-pipe bound: 8 Horner cubics, the exact linear phase term, a quarter-turn sincos and 3 complex
-// multiply-adds per (bin, mode).
+// a6 + a7: fused dense kernel (mbhl_dense.cuh, which documents the work decomposition): interpolates every
+// active mode onto the Fourier bins, sums the modes per bin and accumulates <d|h> and <h|h>
+// (eqs. 2, 3, 11); the template is never written to memory.  Here: its arguments and the device functions it
+// shares with mbhl_template (quarter-turn sincos, interval lookup, one mode's contribution at one bin).
 // ---------------------------------------------------------------------------------------------
 struct DenseArgs {
     const DenseWalker* dw;   // [B]
