@@ -172,3 +172,30 @@ def ladder(n_temps=10, base=2.04807, t_max_inf=True):
     if t_max_inf:
         betas[-1] = 0.0
     return betas
+
+
+def noise_aet(psd, df, seed):
+    """Frequency-domain noise realisation for the three TDI channels (eq. 12; reading G5 of DESIGN.md).
+
+    psd [3, N] one-sided PSD.  The paper draws a modulus N(0, 1/(2 sqrt(df))) sqrt(S_n) and a uniform phase; a normal
+    draw used as a modulus is ambiguous (G5), so this is the standard circular complex Gaussian it approximates:
+    Re and Im independent N(0, S_n / (4 df)), i.e. a Rayleigh modulus sqrt(S_n/(4 df)) sqrt(-2 ln u0) with the
+    uniform phase 2 pi u1 (Box-Muller).  The uniforms come from Philox with counter (bin, channel, stream 3, 0)
+    and key = seed.  Bins with S_n <= 0 or not finite get 0.  Returns complex128 [3, N].
+    """
+    psd = np.asarray(psd, dtype=np.float64)
+    C, N = psd.shape
+    out = np.zeros((C, N), dtype=np.complex128)
+    key = np.array([seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF], dtype=np.uint32)
+    k = np.arange(N, dtype=np.uint32)
+    for c in range(C):
+        ctr = np.stack([k, np.full_like(k, c), np.full_like(k, 3), np.zeros_like(k)], axis=-1)
+        r = philox4x32(ctr, key).astype(np.uint64)
+        u0 = (((r[:, 0] << np.uint64(20)) | (r[:, 1] >> np.uint64(12))).astype(np.float64) + 0.5) * 2.0 ** -52
+        u1 = (((r[:, 2] << np.uint64(20)) | (r[:, 3] >> np.uint64(12))).astype(np.float64) + 0.5) * 2.0 ** -52
+        ok = np.isfinite(psd[c]) & (psd[c] > 0.0)
+        sig = np.sqrt(np.where(ok, psd[c], 0.0) / (4.0 * df))
+        mod = sig * np.sqrt(-2.0 * np.log(u0))
+        ang = 2.0 * math.pi * u1
+        out[c] = mod * np.cos(ang) + 1j * mod * np.sin(ang)
+    return out

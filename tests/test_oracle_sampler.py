@@ -110,3 +110,26 @@ def test_mode_products_are_linear_in_the_modes(table):
     assert np.all(hh >= 0.0) and hh[0] == hh.max()                               # (2,2) dominates
     assert thh <= np.sum(np.sqrt(hh)) ** 2 * (1 + 1e-12)                         # triangle inequality
     assert abs(thh - hh.sum()) > 1e-6 * thh                                      # modes mix
+
+
+def test_noise_realisation_has_the_psd_it_was_drawn_from():
+    # eq. 12 / reading G5: E[4 df |n|^2 / S_n] = 2 per bin, Re and Im independent N(0, S_n/(4 df)), channels independent
+    N, df = 200000, 3.0e-8
+    f = (1.0 + np.arange(N)) * df * 50.0
+    psd = W.scird_psd_aet(f)
+    psd[1, 10] = 0.0
+    psd[2, 11] = np.nan
+    n = S.noise_aet(psd, df, seed=77)
+    assert n[1, 10] == 0.0 and n[2, 11] == 0.0 and np.all(np.isfinite(n.view(np.float64)))
+    good = np.isfinite(psd) & (psd > 0.0)
+    z = np.where(good, n / np.sqrt(np.where(good, psd, 1.0) / (4.0 * df)), 0.0)      # unit-variance Re and Im
+    for c in range(3):
+        zc = z[c][good[c]]
+        assert abs(zc.real.mean()) < 0.01 and abs(zc.imag.mean()) < 0.01
+        assert abs(zc.real.var() - 1.0) < 0.015 and abs(zc.imag.var() - 1.0) < 0.015
+        assert abs(np.mean(zc.real * zc.imag)) < 0.01
+        assert abs(np.mean(np.abs(zc) ** 2) - 2.0) < 0.02                              # 4 df |n|^2 / S_n averages 2
+        assert abs(np.mean(np.abs(zc) ** 4) - 8.0) < 0.3                               # Rayleigh modulus: E r^4 = 8
+    assert abs(np.mean(z[0] * np.conj(z[1]))) < 0.01 and abs(np.mean(z[0] * np.conj(z[2]))) < 0.01
+    # reproducible, and a different seed gives a different stream
+    assert np.array_equal(n, S.noise_aet(psd, df, seed=77)) and not np.array_equal(n, S.noise_aet(psd, df, seed=78))
