@@ -144,6 +144,13 @@ int  mbhl_pt_step(mbhl_pt* pt, int32_t n_steps);                  /* asynchronou
 int  mbhl_pt_state(mbhl_pt* pt, double* theta, double* logL, int64_t* n_accept, int64_t* n_swap);
 void mbhl_pt_free(mbhl_pt* pt);
 
+/* Noise realisation for fabricating data streams (eq. 12; reading G5 of DESIGN.md): for each channel
+ * and bin Re, Im ~ N(0, S_n / (4 df)) independent (the circular Gaussian that eq. 12's "normal modulus, uniform phase"
+ * approximates), drawn by Box-Muller from Philox4x32-10 with key = seed and counter (bin, channel, 3, 0).  psd_AET[3][N]
+ * and out_AET[3][N][2] are device pointers on the current device; bins with S_n <= 0 or non-finite get 0.
+ * Needs no context; asynchronous on `stream` (cudaStream_t, NULL = default stream).  N <= 2^31.            */
+int mbhl_noise(void* stream, const double* psd_AET, int64_t N, double df, uint64_t seed, double* out_AET);
+
 /* Introspection. */
 double  mbhl_data_norm(const mbhl_ctx* ctx);        /* <d|d> computed at init                            */
 int64_t mbhl_num_bins(const mbhl_ctx* ctx);

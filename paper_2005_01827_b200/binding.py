@@ -13,7 +13,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
-SYMBOLS = ("mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
+SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
            "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
            "mbhl_launch_count", "mbhl_last_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
@@ -44,6 +44,7 @@ def lib():
         L.mbhl_loglike_parts.argtypes = [vp, vp, i64, vp, vp, vp]
         L.mbhl_loglike_host.argtypes = [vp, vp, i64, vp]
         L.mbhl_template.argtypes = [vp, vp, i64, vp, i64, vp, i32]
+        L.mbhl_noise.argtypes = [vp, vp, i64, dbl, ctypes.c_uint64, vp]
         L.mbhl_mode_products.argtypes = [vp, vp, i64, vp, vp]
         L.mbhl_loglike_sampled.argtypes = [vp, vp, i64, vp]
         L.mbhl_pt_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32, i32, ctypes.c_uint64, dbl]
@@ -241,3 +242,11 @@ def mbhl_pt_state(pt, T, K, device):
 
 def mbhl_pt_free(pt):
     lib().mbhl_pt_free(pt)
+
+
+def mbhl_noise(psd_AET, df, seed=0, stream=None):
+    """Complex noise realisation [3, N] (torch CUDA complex128) for the one-sided PSD psd_AET [3, N] (torch CUDA)."""
+    n = int(psd_AET.shape[1])
+    out = torch.empty((3, n, 2), dtype=torch.float64, device=psd_AET.device)
+    _check(lib().mbhl_noise(_stream_handle(stream), _ptr(psd_AET), n, float(df), ctypes.c_uint64(int(seed)), _ptr(out)))
+    return torch.view_as_complex(out)

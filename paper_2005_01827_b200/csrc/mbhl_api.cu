@@ -562,6 +562,13 @@ void mbhl_pt_free(mbhl_pt* pt) {
     delete pt;
 }
 
+int mbhl_noise(void* stream, const double* psd_AET, int64_t N, double df, uint64_t seed, double* out_AET) {
+    if (!psd_AET || !out_AET || N < 1 || N > ((int64_t)1 << 31) || !(df > 0.0)) return MBHL_EINVAL;
+    dim3 g((unsigned)((N + 255) / 256), 3);
+    k_noise<<<g, 256, 0, (cudaStream_t)stream>>>(psd_AET, N, df, seed, out_AET);
+    return cudaGetLastError() == cudaSuccess ? MBHL_OK : MBHL_ECUDA;
+}
+
 int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins) {
     if (!ctx) return MBHL_EINVAL;
     unsigned long long h[2];

@@ -69,6 +69,26 @@ __device__ __forceinline__ void uniforms2(uint64_t seed, uint32_t step, uint32_t
     u1 = ((double)b + 0.5) * 0x1p-52;
 }
 
+// Noise realisation of eq. 12 (reading G5): Re, Im ~ N(0, S_n / (4 df)) by Box-Muller from the two
+// uniforms of Philox counter (bin, channel, stream 3, 0); bins with S_n <= 0 or not finite get 0.  out [3][N][2].
+__global__ void k_noise(const double* __restrict__ psd, int64_t N, double df, uint64_t seed, double* __restrict__ out) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (k >= N) return;
+    const double s = psd[c * N + k];
+    double re = 0.0, im = 0.0;
+    if (isfinite(s) && s > 0.0) {
+        double u0, u1;
+        uniforms2(seed, (uint32_t)c, 3u, (uint32_t)k, u0, u1);
+        const double mod = sqrt(s / (4.0 * df)) * sqrt(-2.0 * log(u0));
+        double sn, cs;
+        sincos(2.0 * kPi * u1, &sn, &cs);
+        re = mod * cs;
+        im = mod * sn;
+    }
+    reinterpret_cast<double2*>(out)[c * N + k] = make_double2(re, im);
+}
+
 struct PtState {
     double* theta;       // [T][K][11] sampler coordinates
     double* logl;        // [T][K]

@@ -128,3 +128,17 @@ def test_pt_ensemble_parity(table, small):
     with pytest.raises(M.MbhlError):
         M.mbhl_pt_init(ctx, dev(theta), np.array([1.0, -0.5, 0.0]))
     M.mbhl_free(ctx)
+
+
+def test_noise_realisation_parity():
+    N, df = 100003, 3.0e-8
+    f = (1.0 + np.arange(N)) * df * 100.0
+    psd = W.scird_psd_aet(f)
+    psd[0, 5] = 0.0
+    psd[2, 7] = np.inf
+    ref = S.noise_aet(psd, df, seed=2005018270002)
+    got = M.mbhl_noise(dev(psd), df, seed=2005018270002).cpu().numpy()
+    scale = np.sqrt(np.where(np.isfinite(psd) & (psd > 0), psd, 0.0) / (4.0 * df))
+    assert got[0, 5] == 0.0 and got[2, 7] == 0.0
+    # same uniforms on both sides: only the rounding of log / sqrt / sincos differs
+    assert np.max(np.abs(got - ref) / np.maximum(scale, 1e-300)) <= 1e-13
