@@ -332,3 +332,33 @@ def test_tiny_grids_and_few_knots(table, cfg0):
             ref = L.loglike_parts(table, p[b], f, d, s_, S, 0.0)[2]
             assert abs(ll[b] - ref) <= 1e-6 * (1.0 + abs(ref)), (n, S, b, ll[b], ref)
         M.mbhl_free(ctx)
+
+
+def test_narrow_interval_regime_random_masses(table):
+    # BASELINE config 4 corner: few bins per spline interval (N = 2^14 bins up to 0.1 Hz with S = 1024 knots) and walkers
+    # from 1e5 to 1e8 solar masses in one batch: every path of the dense kernel (staged, knot straddles, scratch, per bin)
+    N = 1 << 14
+    df = 0.1 / N
+    freqs = (1.0 + np.arange(N, dtype=np.float64)) * df
+    psd = W.scird_psd_aet(freqs)
+    params = W.sparse_batch(12, seed_offset=9)
+    params[:, 10] *= (1.0 / df) / (1.33 * W.YEAR_JULIAN_S)          # t_ref as the same fraction of T_obs = 1/df
+    rng = np.random.default_rng(9)
+    data = L.template(table, params[0], freqs, 1024) + W.noise(rng, psd, df)
+    ctx = M.mbhl_init(dev(freqs), dev(data), dev(psd), sparse_points=1024)
+    dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(params))]
+    pairs, bins = M.mbhl_last_work(ctx)
+    assert pairs > 0
+    for b in range(params.shape[0]):
+        rdh, rhh, rll = L.loglike_parts(table, params[b], freqs, data, psd, 1024)
+        assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (b, ll[b], rll)
+        assert abs(hh[b] - rhh) <= 1e-8 * max(rhh, 1e-300), (b, hh[b], rhh)
+    h_gpu = M.mbhl_template(ctx, dev(params[:3])).cpu().numpy()
+    for b in range(3):
+        h_ref = L.template(table, params[b], freqs, 1024)
+        keep = ~edge_mask(table, params[b], freqs, 0.0)
+        for c in range(3):
+            scale = np.max(np.abs(h_ref[c]))
+            if scale > 0:
+                assert np.max(np.abs(h_gpu[b, c][keep] - h_ref[c][keep])) <= 1e-9 * scale
+    M.mbhl_free(ctx)
