@@ -122,3 +122,21 @@ def test_amplitudes_positive_and_inspiral_monotone(table):
             assert np.all(np.diff(I.psi22(f)[1]) > 0.0)        # t(f) strictly increasing up to merger
             assert np.all(I.amp_hat(np.geomspace(1e-5, 0.5, 3000)) > 0.0)
             assert I.gamma2 < 1.0 and 0.5 * I.fRD > F_PHI_INS and I.f_peak > F_AMP_INS
+
+
+def test_higher_mode_table_rows_follow_from_the_leading_pn_multipoles(table):
+    # hm.<lm>.amp / hm.<lm>.dphi (model_data/phenomhm_table.csv, tag "derived") against the textbook leading-PN
+    # time-domain multipoles h_lm = 2 eta M x / R sqrt(16 pi/5) H_lm exp(-i m phi) (Kidder 2008 / Blanchet's review):
+    # the stationary-phase factor of mode m is sqrt(2/m) and the mode content at f > 0 is the transform of
+    # h_{l,-m} = (-1)^l conj(h_lm) (reading G3), so
+    #   c_lm = sqrt(2/m) |H_lm| (mass factors and powers of x stripped),  Delta_lm = (1 - m/2) pi/4 + arg[(-1)^l conj(H_lm)].
+    s = math.sqrt
+    H = {(2, 2): 1.0 + 0.0j, (2, 1): -1j / 3.0, (3, 3): -0.75j * s(15.0 / 14.0), (3, 2): s(5.0 / 7.0) / 3.0 + 0.0j,
+         (4, 4): -8.0 / 9.0 * s(5.0 / 7.0) + 0.0j, (4, 3): -9j / (4.0 * s(70.0))}
+    for (l, m) in MODES:
+        c = s(2.0 / m) * abs(H[(l, m)])
+        z = (-1.0) ** l * np.conj(H[(l, m)])
+        dphi = (1.0 - 0.5 * m) * math.pi / 4.0 + math.atan2(z.imag, z.real)
+        assert abs(table[f"hm.{l}{m}.amp"] - c) < 1e-15, (l, m)
+        d = table[f"hm.{l}{m}.dphi"] - dphi
+        assert abs(d - 2 * math.pi * round(d / (2 * math.pi))) < 1e-14, (l, m)

@@ -96,18 +96,86 @@ def test_p9_frozen_constellation_time_domain_brute_force():
         assert abs(phi_R + 2 * PI * f * (k @ p0)) < 1e-9
 
 
-def test_p12_t_channel_suppressed_at_low_frequency():
+def test_p12_t_channel_vanishes_through_relative_order_x2(table=None):
+    # DESIGN.md section 4 (reading P12) derives it: in X + Y + Z every term that is even in mu = k.n is a function of
+    # the ARM, not of the link direction, and cancels pairwise; the first direction-dependent term of the round-trip
+    # factor sinc[x/2 (1 - mu)] + exp(-ix) sinc[x/2 (1 + mu)] is + i x^3 mu / 12 (x = 2 pi f L/c).  Hence
+    #   T -> (1/sqrt 3) (1 - z^2) (-i x/2) (i x^3/12) 2 [a_31 mu_31 + a_12 mu_12 + a_23 mu_23],  a_sr = n_sr.P.n_sr,
+    # so |T|/|A,E| = c x^3 (SURVEY.md P12 guessed O(x)); the closed form pins the leading coefficient, sign included.
     lam, beta, psi, inc, phi_ref = 1.1, 0.4, 0.7, 1.0, 2.0
-    ratios = []
-    for f in (1e-3, 1e-4, 1e-5):
-        _, (A, E, T) = response.transfer(np.float64(f), np.float64(3.0e6), lam, beta, psi, inc, phi_ref, 2, 2)
+    t = np.float64(3.0e6)
+    k, Pp, Pc = response.source_frame(lam, beta, psi)
+    P = response.mode_polarisation(2, 2, inc, phi_ref, Pp, Pc)
+    _, pL = response.orbit(t)
+    lead = 0.0
+    for (s, r) in ((3, 1), (1, 2), (2, 3)):
+        n = (pL[r] - pL[s]) / ARM_S
+        lead = lead + (n @ P @ n) * (k @ n)
+    ratios, xs = [], []
+    for f, tol in ((1e-3, 0.2), (3e-4, 0.05), (1e-4, 0.02)):
+        x = 2 * PI * f * ARM_S
+        _, (A, E, T) = response.transfer(np.float64(f), t, lam, beta, psi, inc, phi_ref, 2, 2)
+        z = np.exp(-1j * x)
+        T_lead = (1.0 - z * z) * (-0.5j * x) * (1j * x ** 3 / 12.0) * 2.0 * lead / math.sqrt(3.0)
+        assert abs(T / T_lead - 1.0) < tol, (f, T, T_lead)
         ratios.append(abs(T) / math.hypot(abs(A), abs(E)))
-    # For this exactly rigid equilateral constellation the GW response of T vanishes through O(x^2),
-    # x = 2 pi f L/c: |T|/|A,E| = c x^3 with the same c at every f (SURVEY.md P12 guessed O(x))
-    x = [2 * PI * f * ARM_S for f in (1e-3, 1e-4, 1e-5)]
-    c = [r / xi ** 3 for r, xi in zip(ratios, x)]
+        xs.append(x)
+    c = [r / xi ** 3 for r, xi in zip(ratios, xs)]
     assert ratios[0] < 1e-4
-    assert abs(c[0] / c[1] - 1.0) < 0.02 and abs(c[1] / c[2] - 1.0) < 0.02 and c[0] < 0.1
+    assert abs(c[0] / c[1] - 1.0) < 0.05 and abs(c[1] / c[2] - 1.0) < 0.02 and c[0] < 0.1
+
+
+def test_source_frame_is_a_right_handed_transverse_traceless_basis():
+    # pins response.source_frame (O4): k = -n(lambda, beta); P+, Px symmetric, traceless, transverse, normalised and
+    # mutually orthogonal; psi rotates them like a spin-2 pair; (u, v, k) is right handed so that psi is measured from u
+    # towards v as seen along the propagation direction
+    rng = np.random.default_rng(11)
+    for _ in range(8):
+        lam, beta, psi = rng.uniform(0, 2 * PI), math.asin(rng.uniform(-1, 1)), rng.uniform(0, PI)
+        k, Pp, Pc = response.source_frame(lam, beta, psi)
+        nhat = np.array([math.cos(beta) * math.cos(lam), math.cos(beta) * math.sin(lam), math.sin(beta)])
+        assert np.max(np.abs(k + nhat)) < 1e-15 and abs(k @ k - 1.0) < 1e-15
+        for Q in (Pp, Pc):
+            assert np.max(np.abs(Q - Q.T)) < 1e-15 and abs(np.trace(Q)) < 1e-15 and np.max(np.abs(Q @ k)) < 1e-15
+        assert abs(np.sum(Pp * Pp) - 2.0) < 1e-14 and abs(np.sum(Pc * Pc) - 2.0) < 1e-14 and abs(np.sum(Pp * Pc)) < 1e-14
+        _, Pp4, Pc4 = response.source_frame(lam, beta, psi + PI / 4)
+        assert np.max(np.abs(Pp4 - Pc)) < 1e-14 and np.max(np.abs(Pc4 + Pp)) < 1e-14
+        _, Pp2, Pc2 = response.source_frame(lam, beta, psi + PI / 2)
+        assert np.max(np.abs(Pp2 + Pp)) < 1e-14 and np.max(np.abs(Pc2 + Pc)) < 1e-14
+        # at psi = 0: P+ = u u - v v with u along increasing... u = dn/dlambda direction reversed, v = dn/dbeta;
+        # handedness u x v = k
+        _, e_p, e_c = response.source_frame(lam, beta, 0.0)
+        v = np.array([-math.sin(beta) * math.cos(lam), -math.sin(beta) * math.sin(lam), math.cos(beta)])   # d n / d beta
+        u = np.cross(v, k)                                                                                 # so that u x v = k
+        assert np.max(np.abs(e_p - (np.outer(u, u) - np.outer(v, v)))) < 1e-14
+        assert np.max(np.abs(e_c - (np.outer(u, v) + np.outer(v, u)))) < 1e-14
+
+
+def test_mode_polarisation_is_the_positive_frequency_part_of_the_mode_sum():
+    # pins response.mode_polarisation against the DEFINITION (reading G3):
+    #   h+ - i hx = sum_{l, +-m} Y_lm(iota, phi_ref) h_lm(t),  h_{l,-m} = (-1)^l conj(h_lm)   (non-precessing),
+    #   H(t) = h+ P+ + hx Px,
+    # and eq. 5's mode content at f > 0 is, with the Fourier kernel exp(-2 pi i f t) of reading G2, the transform of
+    # h_{l,-m}(t), the member of the pair that carries exp(+i m Omega t).  With a toy h_lm(t) = a exp(-i m Omega t)
+    # the exp(+i m Omega t) coefficient of H(t) (a discrete Fourier projection) must equal P_lm x (-1)^l conj(a).
+    rng = np.random.default_rng(12)
+    nt = 64
+    tt = np.arange(nt) / nt                                  # one period of Omega = 2 pi
+    for (l, m) in MODES:
+        lam, beta, psi = rng.uniform(0, 2 * PI), math.asin(rng.uniform(-1, 1)), rng.uniform(0, PI)
+        inc, phi_ref = math.acos(rng.uniform(-1, 1)), rng.uniform(0, 2 * PI)
+        a = complex(rng.standard_normal(), rng.standard_normal())
+        _, Pp, Pc = response.source_frame(lam, beta, psi)
+        h_pos = a * np.exp(-1j * m * 2 * PI * tt)            # h_{l,m}(t)
+        h_neg = (-1.0) ** l * np.conj(h_pos)                 # h_{l,-m}(t)
+        hc = response.sYlm(l, m, inc, phi_ref) * h_pos + response.sYlm(l, -m, inc, phi_ref) * h_neg
+        hp, hx = hc.real, -hc.imag
+        H = hp[:, None, None] * Pp[None] + hx[:, None, None] * Pc[None]          # [nt, 3, 3], real
+        coeff = np.tensordot(np.exp(-1j * m * 2 * PI * tt), H, axes=(0, 0)) / nt  # projection on exp(+i m Omega t)
+        P = response.mode_polarisation(l, m, inc, phi_ref, Pp, Pc)
+        content = (-1.0) ** l * np.conj(a)                   # amplitude of h_{l,-m}: the f > 0 mode content
+        assert np.max(np.abs(coeff - P * content)) < 1e-12 * abs(a), (l, m)
+        assert np.max(np.abs(P)) > 1e-3                      # not trivially zero
 
 
 def test_spacecraft_relabelling_symmetry():
