@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const doubl
     DenseWalker& d = s_d[warp];
     const int mi = lane % MBHL_NMODE;                  // lanes 6.. repeat the work of lanes 0-5 (identical stores)
     build_walker(params + b * 11, t0, f_min, f_max, S, mode_mask, c, mi, mi + 1);
+    __syncwarp();                                      // lanes L, L + 6, ... stored the same mode: all of them are done
     {
         DenseMode m;
         m.k_lo = 1; m.k_hi = 0; m.ln_flo = 0.0; m.inv_dlog = 0.0;

@@ -176,8 +176,8 @@ __device__ inline void psi_mr_raw(const WalkerConst& c, double f, double* psi, d
     *dpsi = (c.alp[0] + c.alp[1] / (f * f) + c.alp[2] / f14 + c.alp[3] * c.fDM / (c.fDM * c.fDM + x * x)) * c.inveta;
 }
 
-// Aligned Psi_22 and dPsi_22/df.
-__device__ inline void psi22(const WalkerConst& c, double f, double* psi, double* dpsi) {
+// C1-connected Psi_22 and dPsi_22/df before the alignment of reading G4 (reads neither pshift nor tshift).
+__device__ inline void psi22_unaligned(const WalkerConst& c, double f, double* psi, double* dpsi) {
     double p, d;
     if (f < kFPhiIns) {
         psi_ins_raw(c, f, &p, &d);
@@ -190,6 +190,14 @@ __device__ inline void psi22(const WalkerConst& c, double f, double* psi, double
         p += c.C1m + c.C2m * f;
         d += c.C2m;
     }
+    *psi = p;
+    *dpsi = d;
+}
+
+// Aligned Psi_22 and dPsi_22/df.
+__device__ inline void psi22(const WalkerConst& c, double f, double* psi, double* dpsi) {
+    double p, d;
+    psi22_unaligned(c, f, &p, &d);
     *psi = p - c.pshift - c.tshift * (f - c.f_ref);
     *dpsi = d - c.tshift;
 }
@@ -433,6 +441,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
             fdm[mi] = frd[mi] / (2.0 * Q);
         }
     }
+    __syncwarp();                                       // the loop above is lane-divergent (mode_lo/mode_hi differ per lane)
     c.fRD = frd[0];
     c.fDM = fdm[0];
 
@@ -539,10 +548,10 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
         psi_mr_raw(c, c.f_mr, &pr_, &dpr_);
         c.C2m = dpm_ - dpr_;
         c.C1m = pm_ - pr_ - c.C2m * c.f_mr;
-        c.pshift = 0.0;
-        c.tshift = 0.0;
+        // alignment (reading G4) from the unaligned phase, in registers: every field of the shared record is stored
+        // exactly once with the same value by every lane, so no lane can observe a half-built record
         double p0, d0;
-        psi22(c, c.f_ref, &p0, &d0);
+        psi22_unaligned(c, c.f_ref, &p0, &d0);
         c.pshift = p0;
         c.tshift = d0;
     }
@@ -619,8 +628,7 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
             mc.P[2 * e] = 0.5 * (a.re + b.re);
             mc.P[2 * e + 1] = 0.5 * (a.im + b.im);
         }
-        mc.active = 0;
-        mc.f_lo = mc.f_hi = mc.dlog = mc.inv_dlog = mc.ln_flo = 0.0;
+        mc.f_lo = mc.f_hi = mc.dlog = mc.inv_dlog = mc.ln_flo = 0.0;       // active was reset before the __syncwarp at the top
     }
     // bands (O5).  On the inspiral branch of the phase map t_lm(f) = t_22(2 f / m), so the
     // six roots of t_lm(f) = 0 are images of ONE root x0 of t_22 in (2,2) geometric frequency, found once.
