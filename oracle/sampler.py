@@ -199,3 +199,87 @@ def noise_aet(psd, df, seed):
         ang = 2.0 * math.pi * u1
         out[c] = mod * np.cos(ang) + 1j * mod * np.sin(ang)
     return out
+
+
+# ---------------------------------------------------------------------------------------------
+# LISA-frame sampling coordinates ("sampled in the LISA frame and then converted to the SSB frame
+# before waveform generation"; :222 "8 sky location posterior modes in the LISA reference frame").  The paper
+# cites Marsat et al. [40] for the formulas and prints none: DESIGN.md section 4 reading G20 fixes them from
+# the orbit of O4 (oracle/response.py orbit()).
+# ---------------------------------------------------------------------------------------------
+def lisa_frame(alpha):
+    """The 3x3 matrix R whose columns are the LISA-frame basis vectors x_L, y_L, z_L in SSB components (v_SSB = R v_L):
+    R = R_z(alpha) R_y(-pi/3) R_z(-alpha), alpha = Omega_0 t the orbital phase of the constellation
+    centre.  z_L is the normal of the constellation plane (60 degrees from the ecliptic pole, precessing once per
+    year) and the frame also carries the cartwheel rotation: in it the three spacecraft of the O4 orbit sit at the
+    fixed positions (L/sqrt 3)(cos phi_n, sin phi_n, 0), phi_n = pi, -pi/3, +pi/3 (pinned in tests)."""
+    ca, sa = math.cos(alpha), math.sin(alpha)
+    rz = np.array([[ca, -sa, 0.0], [sa, ca, 0.0], [0.0, 0.0, 1.0]])
+    ct, st = 0.5, -math.sqrt(3.0) / 2.0                  # cos, sin of -pi/3
+    ry = np.array([[ct, 0.0, st], [0.0, 1.0, 0.0], [-st, 0.0, ct]])
+    return rz @ ry @ rz.T
+
+
+def _sky_basis(lam, beta):
+    """n (towards the source), u, v of oracle/response.source_frame for sky angles (lam, beta) in any frame."""
+    cl, sl, cb, sb = math.cos(lam), math.sin(lam), math.cos(beta), math.sin(beta)
+    return np.array([cb * cl, cb * sl, sb]), np.array([sl, -cl, 0.0]), np.array([-sb * cl, -sb * sl, cb])
+
+
+def lisa_to_ssb(t_L, lam_L, beta_L, psi_L, t0=0.0):
+    """(t_L, lambda_L, beta_L, psi_L) -> (t_ref, lambda, beta, psi) in the SSB frame (reading G20).
+
+    The frame is taken at the orbital phase alpha = Omega_0 (t0 + t_L) of the LISA-frame time itself, which makes the
+    map explicit.  Sky direction and polarisation basis are rotated as vectors (the wave is the same physical
+    tensor in both frames); t_L is the arrival time of the wavefront at the constellation centre,
+    t_L = t_ref + k.p_0/c with k = -n the propagation vector (a delay tau multiplies by exp(-2 pi i f tau), O0)."""
+    from .constants import AU_S, YEAR_SIDEREAL_S
+    alpha = 2.0 * math.pi / YEAR_SIDEREAL_S * (t0 + t_L)
+    R = lisa_frame(alpha)
+    n_L, u_L, v_L = _sky_basis(lam_L, beta_L)
+    n = R @ n_L
+    beta = math.asin(max(-1.0, min(1.0, n[2])))
+    lam = math.atan2(n[1], n[0]) % (2.0 * math.pi)
+    _, u, v = _sky_basis(lam, beta)
+    u_rot = R @ u_L
+    delta = math.atan2(float(u_rot @ v), float(u_rot @ u))
+    psi = (psi_L + delta) % math.pi
+    p0 = AU_S * np.array([math.cos(alpha), math.sin(alpha), 0.0])
+    t_ref = t_L + float(n @ p0)                          # t_L - k.p_0/c
+    return t_ref, lam, beta, psi
+
+
+def ssb_to_lisa(t_ref, lam, beta, psi, t0=0.0):
+    """Inverse of lisa_to_ssb: the orbital phase depends on t_L itself, so t_L is found by fixed-point iteration
+    (contraction factor Omega_0 R/c = 1e-4)."""
+    from .constants import AU_S, YEAR_SIDEREAL_S
+    n, u, v = _sky_basis(lam, beta)
+    t_L = t_ref
+    for _ in range(60):
+        alpha = 2.0 * math.pi / YEAR_SIDEREAL_S * (t0 + t_L)
+        p0 = AU_S * np.array([math.cos(alpha), math.sin(alpha), 0.0])
+        t_new = t_ref - float(n @ p0)
+        if t_new == t_L:
+            break
+        t_L = t_new
+    alpha = 2.0 * math.pi / YEAR_SIDEREAL_S * (t0 + t_L)
+    R = lisa_frame(alpha)
+    n_L = R.T @ n
+    beta_L = math.asin(max(-1.0, min(1.0, n_L[2])))
+    lam_L = math.atan2(n_L[1], n_L[0]) % (2.0 * math.pi)
+    _, u_L, v_L = _sky_basis(lam_L, beta_L)
+    u_rot = R.T @ u
+    delta = math.atan2(float(u_rot @ v_L), float(u_rot @ u_L))
+    return t_L, lam_L, beta_L, (psi + delta) % math.pi
+
+
+def unpack_sampled_lisa(theta, t0=0.0):
+    """theta [.., 11] = (ln M_T, q, a1, a2, ln D_L, phi_ref, cos iota, lambda_L, sin beta_L, psi_L, ln t_L) with the
+    sky, polarisation and time coordinates in the LISA frame -> physical SSB parameters."""
+    theta = np.asarray(theta, dtype=np.float64)
+    p = unpack_sampled(theta)
+    flat = p.reshape(-1, NDIM)
+    for row in flat:
+        if np.all(np.isfinite(row)):
+            row[10], row[7], row[8], row[9] = lisa_to_ssb(row[10], row[7], row[8], row[9], t0)
+    return flat.reshape(p.shape)

@@ -133,3 +133,101 @@ def test_noise_realisation_has_the_psd_it_was_drawn_from():
     assert abs(np.mean(z[0] * np.conj(z[1]))) < 0.01 and abs(np.mean(z[0] * np.conj(z[2]))) < 0.01
     # reproducible, and a different seed gives a different stream
     assert np.array_equal(n, S.noise_aet(psd, df, seed=77)) and not np.array_equal(n, S.noise_aet(psd, df, seed=78))
+
+
+# ---------------------------------------------------------------------------------------------
+# LISA-frame coordinates (reading G20)
+# ---------------------------------------------------------------------------------------------
+def test_lisa_frame_is_the_constellation_frame_of_the_orbit():
+    # in the frame R(alpha) the spacecraft of the O4 orbit are at rest in the plane z_L = 0, at radius L/sqrt(3) and
+    # angles pi, -pi/3, +pi/3; a wrong tilt sign, a missing cartwheel rotation or a wrong phase fails this
+    from oracle import response
+    from oracle.constants import ARM_S
+    for t in (0.0, 1.1e6, 9.7e6, 2.9e7, 5.5e7):
+        _, pL = response.orbit(np.float64(t))
+        R = S.lisa_frame(response.OMEGA0 * t)
+        assert np.max(np.abs(R @ R.T - np.eye(3))) < 1e-15 and abs(np.linalg.det(R) - 1.0) < 1e-15
+        assert abs(R[2, 2] - 0.5) < 1e-15                                   # plane inclined by 60 degrees
+        for n, phi in ((1, math.pi), (2, -math.pi / 3.0), (3, math.pi / 3.0)):
+            q = R.T @ pL[n]
+            want = ARM_S / math.sqrt(3.0) * np.array([math.cos(phi), math.sin(phi), 0.0])
+            assert np.max(np.abs(q - want)) < 1e-13 * ARM_S, (t, n, q / ARM_S)
+
+
+def test_lisa_to_ssb_rotates_the_wave_tensor_and_round_trips():
+    from oracle import response
+    from oracle.constants import AU_S
+    rng = np.random.default_rng(31)
+    for _ in range(20):
+        t_L = rng.uniform(1e5, 6e7)
+        lam_L, beta_L, psi_L = rng.uniform(0, 2 * math.pi), math.asin(rng.uniform(-1, 1)), rng.uniform(0, math.pi)
+        t_ref, lam, beta, psi = S.lisa_to_ssb(t_L, lam_L, beta_L, psi_L)
+        assert 0.0 <= lam < 2 * math.pi and 0.0 <= psi < math.pi and abs(beta) <= math.pi / 2
+        # the same physical wave: k, P+ and Px built from the LISA-frame angles and rotated to the SSB are those of the SSB angles
+        R = S.lisa_frame(response.OMEGA0 * t_L)
+        kL, PpL, PcL = response.source_frame(lam_L, beta_L, psi_L)
+        k, Pp, Pc = response.source_frame(lam, beta, psi)
+        assert np.max(np.abs(R @ kL - k)) < 1e-14
+        assert np.max(np.abs(R @ PpL @ R.T - Pp)) < 1e-13 and np.max(np.abs(R @ PcL @ R.T - Pc)) < 1e-13
+        # so k.n for every link is the same number in both frames (links are fixed vectors in the LISA frame)
+        _, pL = response.orbit(np.float64(t_L))
+        for (s_, r_) in response.LINKS:
+            n_ssb = pL[r_] - pL[s_]
+            assert abs(k @ n_ssb - kL @ (R.T @ n_ssb)) < 1e-13 * np.linalg.norm(n_ssb)
+        # time: t_L is the arrival of the wavefront at the constellation centre
+        p0, _ = response.orbit(np.float64(t_L))
+        assert abs((t_L - t_ref) - float(k @ p0)) < 4e-16 * t_L + 1e-10 and abs(t_L - t_ref) <= AU_S * (1 + 1e-12)
+        # round trip
+        back = S.ssb_to_lisa(t_ref, lam, beta, psi)
+        assert abs(back[0] - t_L) < 1e-13 * t_L
+        assert abs(math.remainder(back[1] - lam_L, 2 * math.pi)) < 1e-12 and abs(back[2] - beta_L) < 1e-12
+        assert abs(math.remainder(back[3] - psi_L, math.pi)) < 1e-12
+    # a source in the direction of the constellation centre as seen from the Sun is reached R/c EARLIER than the SSB
+    t_L = 4.0e6
+    t_ref, lam, beta, psi = S.lisa_to_ssb(t_L, 0.3, 0.2, 0.1)
+    back = S.ssb_to_lisa(1.0e7, response.OMEGA0 * 1.0e7 % (2 * math.pi), 0.0, 0.4)
+    assert abs((back[0] - 1.0e7) + AU_S) < 1e-3               # alpha moves by Omega_0 R/c = 1e-4 rad in between
+
+
+def test_eight_sky_modes_in_the_lisa_frame():
+    # in the LISA frame the sky posterior has 8 modes, longitudes separated by pi/2, latitudes +-beta_L.
+    # With a frozen constellation at low frequency (x = 2 pi f L/c << 1) the A, E responses of the 8 points
+    # (lambda_L + k pi/2, +-beta_L; the reflected ones with iota -> pi - iota, psi_L -> pi - psi_L) have equal moduli up
+    # to O(x); the same operations applied to SSB angles change them by O(1).
+    from oracle import response
+    from oracle.constants import ARM_S
+    t, f = 1.3e7, 1e-4
+    x = 2 * math.pi * f * ARM_S
+    lam_L, beta_L, psi_L, inc, phi = 1.0, 0.5, 0.7, 1.1, 2.0
+
+    def moduli(lam_L, beta_L, psi_L, inc, frame):
+        if frame == "lisa":
+            _, lam, beta, psi = S.lisa_to_ssb(t, lam_L, beta_L, psi_L)
+        else:
+            lam, beta, psi = lam_L, beta_L, psi_L
+        _, (A, E, T) = response.transfer(np.float64(f), np.float64(t), lam, beta, psi, inc, phi, 2, 2)
+        return abs(A), abs(E)
+
+    for frame, near in (("lisa", True), ("ssb", False)):
+        a0, e0 = moduli(lam_L, beta_L, psi_L, inc, frame)
+        worst = 0.0
+        for k in range(4):
+            a1, e1 = moduli(lam_L + k * math.pi / 2, beta_L, psi_L + k * math.pi / 2, inc, frame)
+            a2, e2 = moduli(lam_L + k * math.pi / 2, -beta_L, math.pi - psi_L + k * math.pi / 2, math.pi - inc, frame)
+            worst = max(worst, abs(a1 / a0 - 1), abs(e1 / e0 - 1), abs(a2 / a0 - 1), abs(e2 / e0 - 1))
+        if near:
+            assert worst < 0.5 * x, (worst, x)
+        else:
+            assert worst > 0.05, worst
+
+
+def test_unpack_sampled_lisa_is_unpack_then_frame_conversion():
+    rng = np.random.default_rng(33)
+    th = rng.uniform(S.PRIOR_LO, S.PRIOR_HI, size=(5, 11))
+    th[:, 10] = np.log(rng.uniform(1e5, 3e7, 5))
+    p = S.unpack_sampled_lisa(th, t0=123.0)
+    q = S.unpack_sampled(th)
+    for b in range(5):
+        t_ref, lam, beta, psi = S.lisa_to_ssb(q[b, 10], q[b, 7], q[b, 8], q[b, 9], 123.0)
+        assert np.array_equal(p[b, [10, 7, 8, 9]], [t_ref, lam, beta, psi])
+        assert np.array_equal(p[b, :7], q[b, :7])
