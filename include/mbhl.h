@@ -55,6 +55,15 @@ extern "C" {
 #define MBHL_ECUDA    -3   /* CUDA runtime error, text in mbhl_last_error                                */
 #define MBHL_ENOWS    -4   /* caller-supplied workspace too small for this batch                         */
 
+/* Coordinates a walker row may be given in (mbhl_loglike_coords, mbhl_unpack_coords, mbhl_pt_init) */
+#define MBHL_COORDS_PHYSICAL      0   /* the 11 physical SSB-frame parameters listed above                            */
+#define MBHL_COORDS_SAMPLED       1   /* the sampler's coordinates: (ln M_T, q, a1, a2, ln D_L, phi_ref,
+                                         cos iota, lambda, sin beta, psi, ln t_ref), sky/polarisation/time in the SSB   */
+#define MBHL_COORDS_SAMPLED_LISA  2   /* the same with (lambda, sin beta, psi, ln t) in the LISA frame:
+                                         what the paper's sampler hands over.  Reading G20 of DESIGN.md: frame of the
+                                         constellation at the orbital phase Omega_0 (t0 + t_L), t_L = arrival time of the
+                                         wavefront at the constellation centre                                          */
+
 #define MBHL_NPARAM   11
 #define MBHL_NMODE     6
 #define MBHL_NQ        8
@@ -62,7 +71,8 @@ extern "C" {
 typedef struct mbhl_ctx mbhl_ctx;     /* opaque; owned by the library, released by mbhl_free */
 
 typedef struct mbhl_config {
-    int32_t  sparse_points;  /* S, knots per mode, >= 8; 0 = default 1024 ("~2^10")          */
+    int32_t  sparse_points;  /* S, knots per mode, 8 <= S <= 2048 (one CTA's shared memory holds a mode's knots
+                                and right-hand sides); 0 = default 1024 ("~2^10")                    */
     uint32_t mode_mask;      /* bit i enables mode i of the order above; 0 = all six                     */
     double   t0;             /* t_coal = t0 + t_ref                                       */
     int64_t  max_batch;      /* hint for the internal workspace; 0 = grow on demand                      */
@@ -116,14 +126,20 @@ int mbhl_set_workspace(mbhl_ctx* ctx, void* dev_ptr, size_t bytes);
 
 /* Per-mode inner products (Table III :292-300): every mode evaluated in isolation against the
  * data.  d_h[B][6] = <d|h_lm>, h_h[B][6] = <h_lm|h_lm> (optimal SNR of the mode alone = sqrt);
- * either may be NULL.  Device pointers; mode order as above; a mode disabled at init gives 0.  B <= 65535.  */
+ * either may be NULL.  Device pointers; mode order as above; a mode disabled at init gives 0.               */
 int mbhl_mode_products(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h);
 
-/* logL for walkers given in the sampler's coordinates (Table I :67-81)
- *   theta[b] = (ln M_T, q, a1, a2, ln D_L, phi_ref, cos iota, lambda, sin beta, psi, ln t_ref),
- * every component uniform between the bounds of Table I.  A walker outside that box gets logL = -inf (zero prior).
- * theta, logL: device pointers.                                                                              */
+/* logL for walkers given in the coordinates `coords` (MBHL_COORDS_*).  For the two sampled forms every component is
+ * uniform between the bounds of Table I and a walker outside that box gets logL = -inf (zero prior);
+ * with MBHL_COORDS_SAMPLED_LISA the box applies to the LISA-frame values.  The conversion to physical SSB parameters
+ * (exp / acos / asin, LISA -> SSB rotation and arrival-time shift) runs inside the per-walker constants kernel.
+ * rows[B][11], logL[B]: device pointers.  mbhl_loglike_sampled(ctx, theta, B, logL) is coords = MBHL_COORDS_SAMPLED.     */
+int mbhl_loglike_coords(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* logL);
 int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* logL);
+
+/* The conversion alone: params_out[B][11] (device) receives the physical SSB parameters of every row (a NaN row for a
+ * walker outside the prior box).  Testing aid; asynchronous on the context's stream.                                    */
+int mbhl_unpack_coords(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* params_out);
 
 /* Parallel-tempered affine-invariant ensemble: n_temps rungs with inverse temperatures
  * betas[t] (host pointer; beta = 0 is T = infinity, :222), n_walkers (even) walkers per rung in the sampler's
@@ -134,10 +150,12 @@ int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* 
  * down (eq. 17).  The target of rung t is prior x L^beta_t with the uniform prior of Table I (:211).  Random
  * numbers: Philox4x32-10 keyed by seed, counter (walker, step, stream), so a run is reproducible.  The
  * ensemble lives on the context's device and stream; nothing returns to the host between steps.
- * n_temps * n_walkers <= 65535.  The context must outlive the ensemble.                                    */
+ * coords = MBHL_COORDS_SAMPLED or MBHL_COORDS_SAMPLED_LISA (the frame the walkers live in).  Every starting walker must
+ * lie inside the prior box and have a finite logL (else MBHL_EINVAL): a walker at logL = -inf could never move on the
+ * beta = 0 rung.  n_temps * n_walkers <= 65535.  The context must outlive the ensemble.                     */
 typedef struct mbhl_pt mbhl_pt;
 int  mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const double* betas, int32_t n_temps,
-                  int32_t n_walkers, uint64_t seed, double stretch_a);
+                  int32_t n_walkers, uint64_t seed, double stretch_a, int32_t coords);
 int  mbhl_pt_step(mbhl_pt* pt, int32_t n_steps);                  /* asynchronous on the context's stream   */
 /* Copies the ensemble out and synchronises: theta[n_temps][n_walkers][11], logL[n_temps][n_walkers] (host or
  * device), accepted moves per rung n_accept[n_temps] and accepted swaps n_swap[n_temps-1] (host).  Any may be NULL. */

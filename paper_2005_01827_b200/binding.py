@@ -13,7 +13,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
-SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
+COORDS_PHYSICAL, COORDS_SAMPLED, COORDS_SAMPLED_LISA = 0, 1, 2        # include/mbhl.h MBHL_COORDS_*
+SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
            "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
            "mbhl_launch_count", "mbhl_last_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
@@ -47,7 +48,9 @@ def lib():
         L.mbhl_noise.argtypes = [vp, vp, i64, dbl, ctypes.c_uint64, vp]
         L.mbhl_mode_products.argtypes = [vp, vp, i64, vp, vp]
         L.mbhl_loglike_sampled.argtypes = [vp, vp, i64, vp]
-        L.mbhl_pt_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32, i32, ctypes.c_uint64, dbl]
+        L.mbhl_loglike_coords.argtypes = [vp, vp, i64, i32, vp]
+        L.mbhl_unpack_coords.argtypes = [vp, vp, i64, i32, vp]
+        L.mbhl_pt_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32, i32, ctypes.c_uint64, dbl, i32]
         L.mbhl_pt_step.argtypes = [vp, i32]
         L.mbhl_pt_state.argtypes = [vp, vp, vp, vp, vp]
         L.mbhl_pt_free.argtypes = [vp]
@@ -216,13 +219,29 @@ def mbhl_loglike_sampled(ctx, theta, logL=None):
     return logL
 
 
-def mbhl_pt_init(ctx, theta0, betas, seed=0, stretch_a=1.15):
+def mbhl_loglike_coords(ctx, rows, coords, logL=None):
+    B = int(rows.shape[0])
+    if logL is None:
+        logL = torch.empty(B, dtype=torch.float64, device=rows.device)
+    _check(lib().mbhl_loglike_coords(ctx, _ptr(rows), B, int(coords), _ptr(logL)), ctx)
+    return logL
+
+
+def mbhl_unpack_coords(ctx, rows, coords):
+    """Physical SSB parameters [B, 11] of rows given in `coords` (NaN rows outside the prior box)."""
+    B = int(rows.shape[0])
+    out = torch.empty((B, NPARAM), dtype=torch.float64, device=rows.device)
+    _check(lib().mbhl_unpack_coords(ctx, _ptr(rows), B, int(coords), _ptr(out)), ctx)
+    return out
+
+
+def mbhl_pt_init(ctx, theta0, betas, seed=0, stretch_a=1.15, coords=COORDS_SAMPLED):
     """theta0 [T, K, 11] (torch CUDA or numpy), betas [T] numpy/host.  Returns the ensemble handle."""
     T, K = int(theta0.shape[0]), int(theta0.shape[1])
     betas = np.ascontiguousarray(betas, dtype=np.float64)
     assert betas.shape == (T,)
     pt = ctypes.c_void_p()
-    _check(lib().mbhl_pt_init(ctx, ctypes.byref(pt), _ptr(theta0), _ptr(betas), T, K, ctypes.c_uint64(int(seed)), float(stretch_a)), ctx)
+    _check(lib().mbhl_pt_init(ctx, ctypes.byref(pt), _ptr(theta0), _ptr(betas), T, K, ctypes.c_uint64(int(seed)), float(stretch_a), int(coords)), ctx)
     return pt
 
 

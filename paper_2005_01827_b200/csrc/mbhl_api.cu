@@ -41,6 +41,8 @@ struct mbhl_ctx {
 
 namespace {
 
+constexpr int64_t kSliceBatch = 32768;   // walkers per pass of the hot path; larger batches are processed in slices
+
 struct WsLayout {
     size_t params, consts, dense, knots, y, coef, partials, dh, hh, logl, total;
 };
@@ -67,15 +69,21 @@ DensePlan dense_plan(int64_t B, int n_chunks) {
     return p;
 }
 
-constexpr int64_t kSliceBatch = 32768;   // walkers per pass of the hot path; larger batches are processed in slices
-
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 int n_chunks_of(int64_t N) { return (int)((N + kChunk - 1) / kChunk); }
 
+// Entries of the partials buffer for any batch b' <= b: b' n_groups(b') is not monotone in b' (G and W grow with the
+// batch), so the workspace is sized by a bound that is: b' ceil(n_chunks / G_max) once G has reached its maximum, and
+// at most 131072 + 8 b' before that (G >= g/2 for g = n_tiles n_chunks / 8192 >= 1, and b' n_chunks < 65536 for g < 1).
+size_t partials_capacity(size_t b, int n_chunks) {
+    return b * (size_t)((n_chunks + kDenseMaxG - 1) / kDenseMaxG) + 131072 + 8 * b;
+}
+
 WsLayout layout(const mbhl_ctx* c, int64_t B) {
     WsLayout L;
     size_t off = 0;
+    if (B > kSliceBatch) B = kSliceBatch;        // larger batches run in slices of kSliceBatch walkers
     const size_t b = (size_t)(B > 0 ? B : 1);
     L.params = off; off += align256(b * MBHL_NPARAM * sizeof(double));
     L.consts = off; off += align256(b * sizeof(WalkerConst));
@@ -83,7 +91,7 @@ WsLayout layout(const mbhl_ctx* c, int64_t B) {
     L.knots = off; off += align256(b * MBHL_NMODE * c->S * sizeof(double));
     L.y = off; off += align256(b * MBHL_NMODE * MBHL_NQ * c->S * sizeof(double));
     L.coef = off; off += align256(b * MBHL_NMODE * (size_t)(c->S - 1) * kCoefStride * sizeof(double));
-    L.partials = off; off += align256(b * (size_t)dense_plan((int64_t)b, n_chunks_of(c->N)).n_groups * 2 * sizeof(double));
+    L.partials = off; off += align256(partials_capacity(b, n_chunks_of(c->N)) * 2 * sizeof(double));
     L.dh = off; off += align256(b * sizeof(double));
     L.hh = off; off += align256(b * sizeof(double));
     L.logl = off; off += align256(b * sizeof(double));
@@ -139,8 +147,29 @@ bool is_device_ptr(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-// Runs the sparse stage (a1-a5) for params already on the device.
-int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, const WsLayout& L, bool with_coef) {
+// k_spline's dynamic shared memory limit is per function and per device, not per context: keep the running maximum
+// so that contexts with different S can coexist (several contexts may be alive at once, mbhl.h).
+int ensure_spline_smem(mbhl_ctx* ctx) {
+    static size_t granted[64] = {0};
+    const size_t need = spline_smem_bytes(ctx->S);
+    const int d = ctx->device & 63;
+    if (granted[d] < need) {
+        CU(cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+        granted[d] = need;
+    }
+    return MBHL_OK;
+}
+
+// Step a1 + a2 for rows[B][11] on the device, given in the coordinates `coords` (MBHL_COORDS_*).
+void run_consts(mbhl_ctx* ctx, const double* rows_dev, int64_t B, int coords, char* base, const WsLayout& L) {
+    k_walker_consts<<<(unsigned)((B + kConstsWarps - 1) / kConstsWarps), 32 * kConstsWarps, 0, ctx->stream>>>(
+        rows_dev, B, coords, ctx->t0, ctx->f_min, ctx->f_max, ctx->S, ctx->mode_mask, ctx->freqs, (int)ctx->N, ctx->df,
+        (WalkerConst*)(base + L.consts), (DenseWalker*)(base + L.dense), (double*)(base + L.params));
+    ctx->launches += 1;
+}
+
+// Runs the sparse stage (a1-a5) for rows already on the device.
+int run_sparse(mbhl_ctx* ctx, const double* rows_dev, int64_t B, int coords, char* base, const WsLayout& L, bool with_coef) {
     WalkerConst* wc = (WalkerConst*)(base + L.consts);
     double* knots = (double*)(base + L.knots);
     double* y = (double*)(base + L.y);
@@ -149,15 +178,15 @@ int run_sparse(mbhl_ctx* ctx, const double* params_dev, int64_t B, char* base, c
     const bool tm = ctx->timing && with_coef;
     if (tm) ctx->ev = ctx->evs[ctx->n_timed % mbhl_ctx::kSlots];
     if (tm) cudaEventRecord(ctx->ev[0], ctx->stream);
-    k_walker_consts<<<(unsigned)((B + kConstsWarps - 1) / kConstsWarps), 32 * kConstsWarps, 0, ctx->stream>>>(params_dev, B, ctx->t0, ctx->f_min, ctx->f_max, S,
-                                                                      ctx->mode_mask, ctx->freqs, (int)ctx->N, ctx->df, wc,
-                                                                      (DenseWalker*)(base + L.dense));
+    run_consts(ctx, rows_dev, B, coords, base, L);
     if (tm) cudaEventRecord(ctx->ev[1], ctx->stream);
     dim3 gs((unsigned)(B * MBHL_NMODE), (unsigned)((S + 127) / 128));
     k_sparse_eval<<<gs, 128, 0, ctx->stream>>>(wc, S, knots, y);
-    ctx->launches += 2;
+    ctx->launches += 1;
     if (tm) cudaEventRecord(ctx->ev[2], ctx->stream);
     if (with_coef) {
+        int rc = ensure_spline_smem(ctx);
+        if (rc != MBHL_OK) return rc;
         k_spline<<<(unsigned)(B * MBHL_NMODE * 2), kSplineThreads, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
         ctx->launches += 1;
     }
@@ -255,7 +284,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         }
         return code;
     };
-    if (ctx->S < 8 || ctx->S > 8192 || !isfinite(ctx->t0)) return cleanup(MBHL_EINVAL);
+    if (ctx->S < 8 || ctx->S > 2048 || !isfinite(ctx->t0)) return cleanup(MBHL_EINVAL);   // mbhl.h: 8 <= S <= 2048
     if (spline_smem_bytes(ctx->S) > 227 * 1024) return cleanup(MBHL_EINVAL);   // S <= ~2170 fits one CTA's shared memory
     if (cudaSetDevice(ctx->device) != cudaSuccess) return cleanup(MBHL_ECUDA);
     if (cudaMemcpyToSymbol(c_table, MBHL_TABLE_HOST, sizeof(double) * MBHL_TABLE_N) != cudaSuccess) return cleanup(MBHL_ECUDA);
@@ -266,8 +295,6 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         if (cudaMemcpyToSymbol(c_prior_lo, lo, sizeof(lo)) != cudaSuccess || cudaMemcpyToSymbol(c_prior_hi, hi, sizeof(hi)) != cudaSuccess)
             return cleanup(MBHL_ECUDA);
     }
-    if (cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)spline_smem_bytes(ctx->S)) != cudaSuccess)
-        return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_spline, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
         cudaFuncSetAttribute(k_dense, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
@@ -361,30 +388,37 @@ int64_t mbhl_num_bins(const mbhl_ctx* ctx) { return ctx ? ctx->N : 0; }
 int32_t mbhl_sparse_points(const mbhl_ctx* ctx) { return ctx ? ctx->S : 0; }
 int64_t mbhl_launch_count(const mbhl_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
-int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h, double* logL) {
+}  // extern "C"
+
+namespace {
+
+// The hot path for rows[B][11] given in the coordinates `coords`; batches above kSliceBatch go in slices, so the
+// workspace stays that of one slice.
+int loglike_impl(mbhl_ctx* ctx, const double* rows, int64_t B, int coords, double* d_h, double* h_h, double* logL) {
     if (!ctx) return MBHL_EINVAL;
-    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
+    if (B < 0 || (B > 0 && !rows) || coords < 0 || coords > 2) return fail(ctx, MBHL_EINVAL, "bad rows/B/coords");
     if (B == 0) return MBHL_OK;
-    if (B > kSliceBatch) {
-        // large batches go in slices, so the workspace stays that of one slice
-        for (int64_t o = 0; o < B; o += kSliceBatch) {
-            const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
-            int rc = mbhl_loglike_parts(ctx, params + o * MBHL_NPARAM, n, d_h ? d_h + o : nullptr, h_h ? h_h + o : nullptr,
-                                        logL ? logL + o : nullptr);
-            if (rc != MBHL_OK) return rc;
-        }
-        return MBHL_OK;
-    }
     CU(cudaSetDevice(ctx->device));
-    char* base;
-    int rc = get_workspace(ctx, B, &base);
-    if (rc != MBHL_OK) return rc;
-    const WsLayout L = layout(ctx, B);
-    rc = run_sparse(ctx, params, B, base, L, true);
-    if (rc != MBHL_OK) return rc;
-    rc = run_dense(ctx, B, base, L, ctx->mode_mask, d_h, h_h, logL, 1, true);
-    if (rc != MBHL_OK) return rc;
+    for (int64_t o = 0; o < B; o += kSliceBatch) {
+        const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
+        char* base;
+        int rc = get_workspace(ctx, n, &base);
+        if (rc != MBHL_OK) return rc;
+        const WsLayout L = layout(ctx, n);
+        rc = run_sparse(ctx, rows + o * MBHL_NPARAM, n, coords, base, L, true);
+        if (rc != MBHL_OK) return rc;
+        rc = run_dense(ctx, n, base, L, ctx->mode_mask, d_h ? d_h + o : nullptr, h_h ? h_h + o : nullptr, logL ? logL + o : nullptr, 1, true);
+        if (rc != MBHL_OK) return rc;
+    }
     return MBHL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mbhl_loglike_parts(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h, double* logL) {
+    return loglike_impl(ctx, params, B, MBHL_COORDS_PHYSICAL, d_h, h_h, logL);
 }
 
 int mbhl_loglike(mbhl_ctx* ctx, const double* params, int64_t B, double* logL) {
@@ -411,7 +445,7 @@ int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, doubl
     double* p_dev = (double*)(base + L.params);
     double* l_dev = (double*)(base + L.logl);
     CU(cudaMemcpyAsync(p_dev, params_host, (size_t)B * MBHL_NPARAM * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    rc = mbhl_loglike_parts(ctx, p_dev, B, nullptr, nullptr, l_dev);
+    rc = loglike_impl(ctx, p_dev, B, MBHL_COORDS_PHYSICAL, nullptr, nullptr, l_dev);
     if (rc != MBHL_OK) return rc;
     CU(cudaMemcpyAsync(logL_host, l_dev, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -420,44 +454,51 @@ int mbhl_loglike_host(mbhl_ctx* ctx, const double* params_host, int64_t B, doubl
 
 int mbhl_mode_products(mbhl_ctx* ctx, const double* params, int64_t B, double* d_h, double* h_h) {
     if (!ctx) return MBHL_EINVAL;
-    if (B < 0 || B > 65535 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B (B <= 65535)");
+    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
     if (B == 0) return MBHL_OK;
     CU(cudaSetDevice(ctx->device));
-    char* base;
-    int rc = get_workspace(ctx, B, &base);
-    if (rc != MBHL_OK) return rc;
-    const WsLayout L = layout(ctx, B);
     const bool tm = ctx->timing;
     ctx->timing = false;
-    rc = run_sparse(ctx, params, B, base, L, true);
-    for (int mi = 0; mi < MBHL_NMODE && rc == MBHL_OK; ++mi)
-        rc = run_dense(ctx, B, base, L, ctx->mode_mask & (1u << mi), d_h ? d_h + mi : nullptr, h_h ? h_h + mi : nullptr, nullptr,
-                       MBHL_NMODE, false);
+    int rc = MBHL_OK;
+    for (int64_t o = 0; o < B && rc == MBHL_OK; o += kSliceBatch) {
+        const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
+        char* base;
+        rc = get_workspace(ctx, n, &base);
+        if (rc != MBHL_OK) break;
+        const WsLayout L = layout(ctx, n);
+        rc = run_sparse(ctx, params + o * MBHL_NPARAM, n, MBHL_COORDS_PHYSICAL, base, L, true);
+        for (int mi = 0; mi < MBHL_NMODE && rc == MBHL_OK; ++mi)
+            rc = run_dense(ctx, n, base, L, ctx->mode_mask & (1u << mi), d_h ? d_h + o * MBHL_NMODE + mi : nullptr,
+                           h_h ? h_h + o * MBHL_NMODE + mi : nullptr, nullptr, MBHL_NMODE, false);
+    }
     ctx->timing = tm;
     return rc;
 }
 
+int mbhl_loglike_coords(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* logL) {
+    if (ctx && B > 0 && !logL) return fail(ctx, MBHL_EINVAL, "logL is null");
+    return loglike_impl(ctx, rows, B, coords, nullptr, nullptr, logL);
+}
+
 int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* logL) {
+    return mbhl_loglike_coords(ctx, theta, B, MBHL_COORDS_SAMPLED, logL);
+}
+
+int mbhl_unpack_coords(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* params_out) {
     if (!ctx) return MBHL_EINVAL;
-    if (B < 0 || (B > 0 && (!theta || !logL))) return fail(ctx, MBHL_EINVAL, "bad theta/logL/B");
-    if (B == 0) return MBHL_OK;
-    if (B > kSliceBatch) {
-        for (int64_t o = 0; o < B; o += kSliceBatch) {
-            const int rc = mbhl_loglike_sampled(ctx, theta + o * MBHL_NPARAM, (B - o < kSliceBatch) ? (B - o) : kSliceBatch, logL + o);
-            if (rc != MBHL_OK) return rc;
-        }
-        return MBHL_OK;
-    }
+    if (B < 0 || (B > 0 && (!rows || !params_out)) || coords < 0 || coords > 2) return fail(ctx, MBHL_EINVAL, "bad rows/B/coords/params_out");
     CU(cudaSetDevice(ctx->device));
-    char* base;
-    int rc = get_workspace(ctx, B, &base);
-    if (rc != MBHL_OK) return rc;
-    const WsLayout L = layout(ctx, B);
-    double* p_dev = (double*)(base + L.params);
-    k_unpack_sampled<<<(unsigned)((B + 127) / 128), 128, 0, ctx->stream>>>(theta, B, p_dev);
-    ctx->launches += 1;
-    CU(cudaGetLastError());
-    return mbhl_loglike_parts(ctx, p_dev, B, nullptr, nullptr, logL);
+    for (int64_t o = 0; o < B; o += kSliceBatch) {
+        const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
+        char* base;
+        int rc = get_workspace(ctx, n, &base);
+        if (rc != MBHL_OK) return rc;
+        const WsLayout L = layout(ctx, n);
+        run_consts(ctx, rows + o * MBHL_NPARAM, n, coords, base, L);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(params_out + o * MBHL_NPARAM, base + L.params, (size_t)n * MBHL_NPARAM * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    return MBHL_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -468,27 +509,29 @@ struct mbhl_pt {
     PtState s = {};
     void* mem = nullptr;
     uint32_t step = 0;
+    int coords = MBHL_COORDS_SAMPLED;
 };
 
 int mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const double* betas_host, int32_t n_temps,
-                 int32_t n_walkers, uint64_t seed, double stretch_a) {
+                 int32_t n_walkers, uint64_t seed, double stretch_a, int32_t coords) {
     if (!ctx || !out) return MBHL_EINVAL;
     *out = nullptr;
     if (!theta0 || !betas_host || n_temps < 1 || n_walkers < 2 || (n_walkers & 1) || !(stretch_a > 1.0) ||
-        (int64_t)n_temps * n_walkers > 65535)
-        return fail(ctx, MBHL_EINVAL, "mbhl_pt_init: need n_temps >= 1, an even n_walkers >= 2, n_temps * n_walkers <= 65535, a > 1");
+        (int64_t)n_temps * n_walkers > 65535 || (coords != MBHL_COORDS_SAMPLED && coords != MBHL_COORDS_SAMPLED_LISA))
+        return fail(ctx, MBHL_EINVAL, "mbhl_pt_init: need n_temps >= 1, an even n_walkers >= 2, n_temps * n_walkers <= 65535, a > 1, sampled coords");
     for (int t = 0; t < n_temps; ++t)
         if (!(betas_host[t] >= 0.0) || !isfinite(betas_host[t])) return fail(ctx, MBHL_EINVAL, "mbhl_pt_init: betas must be finite and >= 0");
     CU(cudaSetDevice(ctx->device));
     mbhl_pt* pt = new (std::nothrow) mbhl_pt();
     if (!pt) return MBHL_ENOMEM;
     pt->ctx = ctx;
+    pt->coords = coords;
     const size_t T = (size_t)n_temps, K = (size_t)n_walkers, H = K / 2;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align256(bytes); return o; };
     const size_t o_theta = take(T * K * MBHL_NPARAM * 8), o_logl = take(T * K * 8), o_betas = take(T * 8);
-    const size_t o_pth = take(T * H * MBHL_NPARAM * 8), o_ppar = take(T * H * MBHL_NPARAM * 8), o_pl = take(T * H * 8), o_pz = take(T * H * 8);
-    const size_t o_acc = take(T * 8), o_swp = take(T * 8), o_tmp = take(T * K * MBHL_NPARAM * 8);
+    const size_t o_pth = take(T * H * MBHL_NPARAM * 8), o_pl = take(T * H * 8), o_pz = take(T * H * 8);
+    const size_t o_acc = take(T * 8), o_swp = take(T * 8);
     if (cudaMalloc(&pt->mem, off) != cudaSuccess) {
         cudaGetLastError();
         delete pt;
@@ -497,7 +540,7 @@ int mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const doubl
     char* m = (char*)pt->mem;
     PtState& s = pt->s;
     s.theta = (double*)(m + o_theta); s.logl = (double*)(m + o_logl); s.betas = (double*)(m + o_betas);
-    s.prop_theta = (double*)(m + o_pth); s.prop_params = (double*)(m + o_ppar); s.prop_logl = (double*)(m + o_pl);
+    s.prop_theta = (double*)(m + o_pth); s.prop_logl = (double*)(m + o_pl);
     s.prop_z = (double*)(m + o_pz); s.n_accept = (unsigned long long*)(m + o_acc); s.n_swap = (unsigned long long*)(m + o_swp);
     s.T = n_temps; s.K = n_walkers; s.a = stretch_a; s.seed = seed;
     int rc = MBHL_OK;
@@ -506,13 +549,17 @@ int mbhl_pt_init(mbhl_ctx* ctx, mbhl_pt** out, const double* theta0, const doubl
         cudaMemcpyAsync(s.betas, betas_host, T * 8, cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
         cudaMemsetAsync(s.n_accept, 0, 2 * align256(T * 8), ctx->stream) != cudaSuccess)
         return bail(fail(ctx, MBHL_ECUDA, "mbhl_pt_init: copies"));
-    // log-likelihood of the starting positions (walkers outside the prior box get -inf)
-    double* tmp = (double*)(m + o_tmp);
-    k_unpack_sampled<<<(unsigned)((T * K + 127) / 128), 128, 0, ctx->stream>>>(s.theta, (int64_t)(T * K), tmp);
-    ctx->launches += 1;
-    rc = mbhl_loglike_parts(ctx, tmp, (int64_t)(T * K), nullptr, nullptr, s.logl);
+    // log-likelihood of the starting positions.  Every walker must start inside the prior box of Table I with a finite
+    // logL: with beta = 0 on the hottest rung a walker at logL = -inf would give 0 x (-inf) = NaN in the
+    // acceptance ratio and could never move; accepted proposals always have a finite logL, so this holds for the whole run.
+    rc = loglike_impl(ctx, s.theta, (int64_t)(T * K), coords, nullptr, nullptr, s.logl);
     if (rc != MBHL_OK) return bail(rc);
-    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return bail(fail(ctx, MBHL_ECUDA, "mbhl_pt_init: sync"));
+    std::vector<double> l0(T * K);
+    if (cudaMemcpyAsync(l0.data(), s.logl, T * K * 8, cudaMemcpyDeviceToHost, ctx->stream) != cudaSuccess ||
+        cudaStreamSynchronize(ctx->stream) != cudaSuccess)
+        return bail(fail(ctx, MBHL_ECUDA, "mbhl_pt_init: sync"));
+    for (size_t i = 0; i < T * K; ++i)
+        if (!isfinite(l0[i])) return bail(fail(ctx, MBHL_EINVAL, "mbhl_pt_init: a starting walker lies outside the prior box or has no finite logL"));
     *out = pt;
     return MBHL_OK;
 }
@@ -526,7 +573,7 @@ int mbhl_pt_step(mbhl_pt* pt, int32_t n_steps) {
     for (int it = 0; it < n_steps; ++it, ++pt->step) {
         for (int half = 0; half < 2; ++half) {
             k_pt_propose<<<(M + 127) / 128, 128, 0, ctx->stream>>>(s, half, 2u * pt->step + (uint32_t)half);
-            int rc = mbhl_loglike_parts(ctx, s.prop_params, M, nullptr, nullptr, s.prop_logl);
+            int rc = loglike_impl(ctx, s.prop_theta, M, pt->coords, nullptr, nullptr, s.prop_logl);
             if (rc != MBHL_OK) return rc;
             k_pt_accept<<<(M + 127) / 128, 128, 0, ctx->stream>>>(s, half, 2u * pt->step + (uint32_t)half);
             ctx->launches += 2;
@@ -584,33 +631,36 @@ int mbhl_template(mbhl_ctx* ctx, const double* params, int64_t B, const double* 
     if (!ctx) return MBHL_EINVAL;
     if (B < 0 || (B > 0 && (!params || !out_AET))) return fail(ctx, MBHL_EINVAL, "bad template arguments");
     if (!freqs_out) { freqs_out = ctx->freqs; Nout = ctx->N; }
-    if (Nout < 0 || B > 65535) return fail(ctx, MBHL_EINVAL, "bad Nout or B > 65535");
+    if (Nout < 0) return fail(ctx, MBHL_EINVAL, "bad Nout");
     if (B == 0 || Nout == 0) return MBHL_OK;
     CU(cudaSetDevice(ctx->device));
-    char* base;
-    int rc = get_workspace(ctx, B, &base);
-    if (rc != MBHL_OK) return rc;
-    const WsLayout L = layout(ctx, B);
-    rc = run_sparse(ctx, params, B, base, L, direct == 0);
-    if (rc != MBHL_OK) return rc;
-    dim3 g((unsigned)((Nout + 127) / 128), (unsigned)B);
-    k_template<<<g, 128, 0, ctx->stream>>>((const WalkerConst*)(base + L.consts), (const double*)(base + L.knots),
-                                           (const double*)(base + L.coef), ctx->S, freqs_out, Nout, out_AET, direct ? 1 : 0);
-    ctx->launches += 1;
-    CU(cudaGetLastError());
+    for (int64_t o = 0; o < B; o += kSliceBatch) {       // slices, like the likelihood calls
+        const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
+        char* base;
+        int rc = get_workspace(ctx, n, &base);
+        if (rc != MBHL_OK) return rc;
+        const WsLayout L = layout(ctx, n);
+        rc = run_sparse(ctx, params + o * MBHL_NPARAM, n, MBHL_COORDS_PHYSICAL, base, L, direct == 0);
+        if (rc != MBHL_OK) return rc;
+        dim3 g((unsigned)((Nout + 127) / 128), (unsigned)n);
+        k_template<<<g, 128, 0, ctx->stream>>>((const WalkerConst*)(base + L.consts), (const double*)(base + L.knots),
+                                               (const double*)(base + L.coef), ctx->S, freqs_out, Nout, out_AET + o * 6 * Nout, direct ? 1 : 0);
+        ctx->launches += 1;
+        CU(cudaGetLastError());
+    }
     return MBHL_OK;
 }
 
 int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, double* y, double* coef) {
     if (!ctx) return MBHL_EINVAL;
-    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
+    if (B < 0 || B > kSliceBatch || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B (mbhl_sparse takes B <= 32768)");
     if (B == 0) return MBHL_OK;
     CU(cudaSetDevice(ctx->device));
     char* base;
     int rc = get_workspace(ctx, B, &base);
     if (rc != MBHL_OK) return rc;
     const WsLayout L = layout(ctx, B);
-    rc = run_sparse(ctx, params, B, base, L, true);
+    rc = run_sparse(ctx, params, B, MBHL_COORDS_PHYSICAL, base, L, true);
     if (rc != MBHL_OK) return rc;
     if (ctx->timing) {   // stages 3 and 4 (dense, reduce) do not run here: zero-length intervals
         for (int i = 3; i < 6; ++i) cudaEventRecord(ctx->ev[i], ctx->stream);

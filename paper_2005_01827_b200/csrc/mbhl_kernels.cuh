@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include "mbhl_model.cuh"
+#include "mbhl_sampler.cuh"   // sampler coordinates, LISA frame, stretch move, temperature swaps
 
 namespace mbhl {
 
@@ -111,10 +112,15 @@ __device__ inline int last_bin_le(const double* __restrict__ f, int N, double f0
 
 constexpr int kConstsWarps = 4;      // walkers per CTA of k_walker_consts (one warp each)
 
-__global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const double* __restrict__ params, int64_t B, double t0, double f_min,
+// rows [B][11]: the walkers in the coordinates named by `coords` (mbhl.h MBHL_COORDS_*): physical SSB parameters, the
+// sampler's coordinates (Table I box :67-81 -> outside it the walker is invalid, logL = -inf), or the
+// sampler's coordinates with (lambda, sin beta, psi, ln t) in the LISA frame (reading G20).  The
+// conversion runs in registers here, so a sampler hands over raw walker coordinates and no extra kernel runs.
+// params_out (may be null): the physical SSB parameters the walker was converted to (NaN row if outside the box).
+__global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const double* __restrict__ rows, int64_t B, int coords, double t0, double f_min,
                                                       double f_max, int S, uint32_t mode_mask, const double* __restrict__ freqs,
                                                       int N, double df, WalkerConst* __restrict__ out,
-                                                      DenseWalker* __restrict__ dw) {
+                                                      DenseWalker* __restrict__ dw, double* __restrict__ params_out) {
     __shared__ WalkerConst s_c[kConstsWarps];
     __shared__ DenseWalker s_d[kConstsWarps];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -122,8 +128,25 @@ __global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const doubl
     if (b >= B) return;
     WalkerConst& c = s_c[warp];
     DenseWalker& d = s_d[warp];
+    double p[MBHL_NPARAM];
+#pragma unroll
+    for (int i = 0; i < MBHL_NPARAM; ++i) p[i] = rows[b * MBHL_NPARAM + i];
+    if (coords != 0) {
+        double th[MBHL_NPARAM];
+#pragma unroll
+        for (int i = 0; i < MBHL_NPARAM; ++i) th[i] = p[i];
+        unpack_sampled(th, p);                          // NaN row outside the box of Table I
+        if (coords == 2 && isfinite(p[10])) lisa_to_ssb(t0, p[10], p[7], p[8], p[9]);
+    }
+    __syncwarp();                                       // rows and params_out may be the same buffer: every lane has read its row
+    if (params_out != nullptr && lane < MBHL_NPARAM) {
+        double v = p[0];
+#pragma unroll
+        for (int i = 1; i < MBHL_NPARAM; ++i) v = (lane == i) ? p[i] : v;
+        params_out[b * MBHL_NPARAM + lane] = v;
+    }
     const int mi = lane % MBHL_NMODE;                  // lanes 6.. repeat the work of lanes 0-5 (identical stores)
-    build_walker(params + b * 11, t0, f_min, f_max, S, mode_mask, c, mi, mi + 1);
+    build_walker(p, t0, f_min, f_max, S, mode_mask, c, mi, mi + 1);
     __syncwarp();                                      // lanes L, L + 6, ... stored the same mode: all of them are done
     {
         DenseMode m;
@@ -511,7 +534,6 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
 }  // namespace mbhl
 
 #include "mbhl_dense.cuh"   // a6 + a7: the fused dense kernel
-#include "mbhl_sampler.cuh" // sampler coordinates, stretch move, temperature swaps
 
 namespace mbhl {
 

@@ -1,7 +1,9 @@
 // mbhl_sampler.cuh - sampler-side steps next to the likelihood (section II.B).
 //
-//   k_unpack_sampled   sampler coordinates (Table I :67-81) -> physical parameters;
+//   unpack_sampled     sampler coordinates (Table I :67-81) -> physical parameters;
 //                      a walker outside the prior box becomes a NaN row, which the hot path maps to logL = -inf
+//   lisa_to_ssb        LISA-frame (lambda, beta, psi, t) -> SSB (reading G20)
+//                      (both run inside k_walker_consts, in registers: no separate kernel)
 //   k_pt_propose       stretch move, eqs. 14-15, a = 1.15 (:222): one thread per moving walker
 //   k_pt_accept        eq. 16 on the tempered density prior x L^beta (:211)
 //   k_pt_swap          eq. 17: swaps between adjacent temperatures, hottest pair first
@@ -36,15 +38,43 @@ __device__ __forceinline__ void unpack_sampled(const double* th, double* p) {
     p[6] = acos(th[6]); p[7] = th[7]; p[8] = asin(th[8]); p[9] = th[9]; p[10] = exp(th[10]);
 }
 
-__global__ void k_unpack_sampled(const double* __restrict__ theta, int64_t B, double* __restrict__ params) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    double th[MBHL_NPARAM], p[MBHL_NPARAM];
-#pragma unroll
-    for (int i = 0; i < MBHL_NPARAM; ++i) th[i] = theta[b * MBHL_NPARAM + i];
-    unpack_sampled(th, p);
-#pragma unroll
-    for (int i = 0; i < MBHL_NPARAM; ++i) params[b * MBHL_NPARAM + i] = p[i];
+// LISA-frame coordinates -> SSB (reading G20).  The frame is that of the constellation at the
+// orbital phase alpha = Omega_0 (t0 + t_L): R = R_z(alpha) R_y(-pi/3) R_z(-alpha), written out entry by entry (the three
+// spacecraft are at rest in it).  Sky direction and polarisation basis rotate as vectors; t_L is the arrival time of the
+// wavefront at the constellation centre: t_ref = t_L - k.p_0/c = t_L + n.p_0/c.  lambda wraps mod 2 pi, psi mod pi.
+__device__ __forceinline__ void lisa_to_ssb(double t0, double& t, double& lam, double& beta, double& psi) {
+    double sa, ca;
+    sincos(kOmega0 * (t0 + t), &sa, &ca);
+    const double ct = 0.5, st = -0.86602540378443864676;        // cos, sin of the tilt -pi/3
+    const double R00 = ct * ca * ca + sa * sa, R01 = ca * sa * (ct - 1.0), R02 = ca * st;
+    const double R10 = R01, R11 = ct * sa * sa + ca * ca, R12 = sa * st;
+    const double R20 = -st * ca, R21 = -st * sa, R22 = ct;
+    double sl, cl, sb, cb;
+    sincos(lam, &sl, &cl);
+    sincos(beta, &sb, &cb);
+    const double nL[3] = {cb * cl, cb * sl, sb}, uL[3] = {sl, -cl, 0.0};
+    const double n0 = R00 * nL[0] + R01 * nL[1] + R02 * nL[2];
+    const double n1 = R10 * nL[0] + R11 * nL[1] + R12 * nL[2];
+    const double n2 = R20 * nL[0] + R21 * nL[1] + R22 * nL[2];
+    const double u0 = R00 * uL[0] + R01 * uL[1], u1 = R10 * uL[0] + R11 * uL[1], u2 = R20 * uL[0] + R21 * uL[1];
+    const double beta_s = asin(fmax(-1.0, fmin(1.0, n2)));
+    double lam_s = atan2(n1, n0);
+    if (lam_s < 0.0) lam_s += kTwoPi;
+    if (lam_s >= kTwoPi) lam_s -= kTwoPi;
+    double sls, cls, sbs, cbs;
+    sincos(lam_s, &sls, &cls);
+    sincos(beta_s, &sbs, &cbs);
+    // SSB polarisation basis at (lam_s, beta_s): u = (sin, -cos, 0), v = (-sin b cos l, -sin b sin l, cos b)
+    const double uu = u0 * sls - u1 * cls;
+    const double uv = -u0 * sbs * cls - u1 * sbs * sls + u2 * cbs;
+    double ps = psi + atan2(uv, uu);
+    ps -= floor(ps / kPi) * kPi;
+    if (ps >= kPi) ps -= kPi;
+    if (ps < 0.0) ps += kPi;
+    t = t + kAuS * (n0 * ca + n1 * sa);
+    lam = lam_s;
+    beta = beta_s;
+    psi = ps;
 }
 
 // Philox4x32-10: counter c[4], key k[2]
@@ -93,8 +123,7 @@ struct PtState {
     double* theta;       // [T][K][11] sampler coordinates
     double* logl;        // [T][K]
     double* betas;       // [T]
-    double* prop_theta;  // [T][K/2][11] proposals (sampler coordinates)
-    double* prop_params; // [T][K/2][11] proposals (physical, NaN rows outside the prior)
+    double* prop_theta;  // [T][K/2][11] proposals (sampler coordinates; the hot path converts them itself)
     double* prop_logl;   // [T][K/2]
     double* prop_z;      // [T][K/2]
     unsigned long long* n_accept;   // [T]
@@ -120,15 +149,9 @@ __global__ void k_pt_propose(PtState s, int half, uint32_t step) {
     const int j = 2 * jj + (1 - half);                                       // partner from the other half
     const double* xk = s.theta + ((int64_t)t * s.K + k) * MBHL_NPARAM;
     const double* xj = s.theta + ((int64_t)t * s.K + j) * MBHL_NPARAM;
-    double y[MBHL_NPARAM], p[MBHL_NPARAM];
 #pragma unroll
-    for (int d = 0; d < MBHL_NPARAM; ++d) y[d] = __dadd_rn(xj[d], __dmul_rn(z, __dadd_rn(xk[d], -xj[d])));   // eq. 14, no contraction
-    unpack_sampled(y, p);
-#pragma unroll
-    for (int d = 0; d < MBHL_NPARAM; ++d) {
-        s.prop_theta[(int64_t)idx * MBHL_NPARAM + d] = y[d];
-        s.prop_params[(int64_t)idx * MBHL_NPARAM + d] = p[d];
-    }
+    for (int d = 0; d < MBHL_NPARAM; ++d)                                                                   // eq. 14, no contraction
+        s.prop_theta[(int64_t)idx * MBHL_NPARAM + d] = __dadd_rn(xj[d], __dmul_rn(z, __dadd_rn(xk[d], -xj[d])));
     s.prop_z[idx] = z;
 }
 

@@ -234,6 +234,30 @@ def test_host_pointers_at_init_and_workspace_api(table, cfg0):
     M.mbhl_free(ctx_h)
 
 
+def test_two_live_contexts_with_different_sparse_sizes(table, cfg0):
+    # k_spline's dynamic shared memory limit is per function, not per context (ADVICE): a second context with a smaller S
+    # must not break the first one
+    big = make_ctx(cfg0)                                             # S = 256
+    p = dev(cfg0["params"])
+    a = M.mbhl_loglike(big, p).cpu().numpy()
+    n = 4 * 512
+    small = M.mbhl_init(dev(cfg0["freqs"][:n]), dev(cfg0["data"][:, :n]), dev(cfg0["psd"][:, :n]), sparse_points=16)
+    M.mbhl_loglike(small, p)
+    huge = M.mbhl_init(dev(cfg0["freqs"][:n]), dev(cfg0["data"][:, :n]), dev(cfg0["psd"][:, :n]), sparse_points=2048)
+    assert torch.isfinite(M.mbhl_loglike(huge, p)).all()
+    assert np.array_equal(M.mbhl_loglike(big, p).cpu().numpy(), a)
+    assert torch.isfinite(M.mbhl_loglike(small, p)).all()
+    for c in (big, small, huge):
+        M.mbhl_free(c)
+    with pytest.raises(M.MbhlError, match="invalid argument"):
+        M.mbhl_init(dev(cfg0["freqs"][:n]), dev(cfg0["data"][:, :n]), dev(cfg0["psd"][:, :n]), sparse_points=2049)
+    # workspace sizing is monotone in B and covers one slice for any larger batch (ADVICE)
+    c = make_ctx(cfg0)
+    sizes = [M.mbhl_workspace_bytes(c, b) for b in (1, 2, 7, 8, 9, 64, 1000, 32768, 40000, 10 ** 6)]
+    assert all(x <= y for x, y in zip(sizes, sizes[1:])) and sizes[-1] == sizes[-3]
+    M.mbhl_free(c)
+
+
 def test_init_rejects_bad_grids(cfg0):
     f = cfg0["freqs"][:1000].copy()
     d = np.ascontiguousarray(cfg0["data"][:, :1000])
