@@ -28,12 +28,29 @@ if ROOT not in sys.path:
 METRIC = "log-likelihoods/sec"
 FLOP_PER_PAIR = 113.0     # per (walker, bin, active mode)
 FLOP_PER_BIN = 40.0       # per (walker, active bin) epilogue
-# the roofline numerator is the LESSER of the table count and what ncu counts as executed.  Since the
-# linear phase term is folded into the spline records and a knot inside a warp tile costs one pass, the kernel executes
-# fewer FP64 operations than the table: ncu (profiles/r01_dense_c2_final_ncu.txt) counts 2 x 6.683e11 DFMA + 6.16e10 DADD
-# + 6.15e10 DMUL = 1.4598e12 FLOPs per config-2 launch against 1.6038e12 from the table.
-EXECUTED_OVER_TABLE_FLOPS = 1.4598e12 / 1.6038e12
+# the roofline numerator is the LESSER of the table count and what the kernel EXECUTES.  The executed
+# count is taken per run from the tallies k_dense keeps (mbhl_last_dense_work: evaluator calls, each 4 bins x 32 lanes,
+# in band or not) times the FP64 operations of one evaluation as written in csrc/mbhl_dense.cuh:
+#   one mode at one bin: 48 DFMA + 4 DADD + 4 DMUL = 104 FLOPs (+1 DMUL when the amplitude is gated),
+#   epilogue per (walker, bin): 12 DFMA + 3 DMUL + 2.75 DADD (per-lane sums and the shuffle tree, per bin) = 29.75 FLOPs.
+# profiles/r02_dense_flop_check.md compares this count with ncu's sm__sass_thread_inst_executed_op_d*_pred_on.
+F_EVAL, F_EVAL_GATED, F_EPI = 104.0, 105.0, 29.75
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x 2 x max SM clock
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_dense launch from the committed `ncu --set full` captures, by config
+DENSE_TRAFFIC = {2: (2.04e9, "profiles/r01_dense_c2_final_ncu.txt")}
+
+
+def executed_flops(counts):
+    """FP64 FLOPs k_dense executed, from its own tallies (uniform, gated, per-bin-record calls; lane evaluations; epilogues)."""
+    n_uni, n_gat, n_rec, n_lane, n_epi = counts
+    return 128.0 * (F_EVAL * n_uni + F_EVAL_GATED * (n_gat + n_rec) + F_EPI * n_epi) + F_EVAL_GATED * n_lane
+
+
+def dense_numerator(pairs, bins, counts):
+    """(FLOPs for the roofline numerator, table FLOPs, executed FLOPs): the lesser of the two."""
+    table = FLOP_PER_PAIR * pairs + FLOP_PER_BIN * bins
+    execd = executed_flops(counts)
+    return min(table, execd), table, execd
 
 
 class ClockSampler:
@@ -75,44 +92,88 @@ def workload_name(cfg, B, N, S):
     return f"BASELINE.json configs[{cfg}]: B={B} walkers x 6 PhenomHM modes, S={S} sparse knots/mode, N={N} dense bins, A/E/T"
 
 
-def oracle_sample(cfg, n_bins=None):
-    """Builds the workload with the oracle's injections and returns (workload, sample walker indices)."""
-    from oracle import likelihood as L
-    from oracle.constants import load_model_table
-    from paper_2005_01827_b200 import workloads as W
-    table = load_model_table()
-    wl = W.build(cfg, lambda p, f, S: L.template(table, p, f, S), n_bins=n_bins)
-    B = wl["params"].shape[0]
-    idx = [0, B // 2, B - 1] if cfg == 2 else ([0, 1] if cfg == 0 else [0])
-    return table, wl, idx
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
 
 
-def time_oracle(table, wl, idx):
+_ORACLE = {}
+
+
+def _oracle_one(b):
     from oracle import likelihood as L
-    t0 = time.perf_counter()
-    for b in idx:
-        L.loglike_parts(table, wl["params"][b], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])
-    return time.perf_counter() - t0
+    wl = _ORACLE["wl"]
+    return L.loglike_parts(_ORACLE["table"], wl["params"][b], wl["freqs"], wl["data"], wl["psd"], wl["S"], wl["t0"])[2]
+
+
+def _oracle_template(args):
+    from oracle import likelihood as L
+    p, f, S = args
+    return L.template(_ORACLE["table"], p, f, S)
+
+
+class OraclePool:
+    """The oracle, as it stands, over all host cores: one walker per worker process (fork; must be created before this
+    process touches CUDA).  The workload is built once with the oracle's own injections and inherited by the workers."""
+
+    def __init__(self, cfg):
+        import multiprocessing as mp
+        from oracle.constants import load_model_table
+        from paper_2005_01827_b200 import workloads as W
+        self.cores = host_cores()
+        _ORACLE["table"] = load_model_table()
+        ctx = mp.get_context("fork")
+        with ctx.Pool(min(self.cores, 3)) as pool0:     # the injections (up to three templates) in parallel too
+            cache = {}
+
+            def tf(p, f, S):
+                return cache[tuple(p)]
+            # W.build asks for the injection templates one by one: precompute them in parallel from a dry run
+            dry = []
+            W.build(cfg, lambda p, f, S: (dry.append((p.copy(), f, S)), np.zeros((3, f.size), dtype=np.complex128))[1], with_noise=False)
+            for (p, f, S), h in zip(dry, pool0.map(_oracle_template, dry)):
+                cache[tuple(p)] = h
+            _ORACLE["wl"] = W.build(cfg, tf)
+        self.wl = _ORACLE["wl"]
+        self.pool = ctx.Pool(self.cores)
+
+    def sample(self, n):
+        B = self.wl["params"].shape[0]
+        return sorted(set(int(round(v)) for v in np.linspace(0, B - 1, min(n, B))))
+
+    def time(self, idx):
+        t0 = time.perf_counter()
+        out = self.pool.map(_oracle_one, idx, chunksize=1)
+        return time.perf_counter() - t0, out
+
+    def close(self):
+        self.pool.terminate()
+        self.pool.join()
 
 
 def run_reference(args):
-    """--impl reference: the oracle, as it stands, on this box's host cores (one process, numpy)."""
+    """--impl reference: the oracle, as it stands, on this box's host cores (one walker per process, numpy)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    table, wl, idx = oracle_sample(args.config)
+    pool = OraclePool(args.config)
+    wl = pool.wl
     B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
-    for _ in range(args.warmup):
-        time_oracle(table, wl, idx[:1])
-    t = sum(time_oracle(table, wl, idx) for _ in range(args.steps))
+    idx = pool.sample(min(16, max(3, pool.cores)))
+    for _ in range(min(args.warmup, 1)):
+        pool.time(idx[:pool.cores])
+    t = sum(pool.time(idx)[0] for _ in range(args.steps))
+    pool.close()
     value = len(idx) * args.steps / t
-    sample = f"walkers {idx} of the batch per step (one per injection group), full grid, single numpy process"
+    sample = f"{len(idx)} walkers {idx} of the batch per step (spread over the injection groups), full grid, one walker per process on {pool.cores} cores"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "logL/s", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, B, N, S), "sample": sample},
-        "cpu_baseline": {"value": value, "unit": "logL/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "logL/s", "cores": pool.cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "logL/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -211,7 +272,7 @@ def run_dense_sweep(args):
     hbm, _ = _hbm_peak()
     all_params = W.sparse_batch(4096, seed_offset=4)
     rng = np.random.default_rng(W.SEED0 + 4)
-    for logn in (16, 18, 20, 22, 23):
+    for logn in ((args.logn,) if args.logn else (16, 18, 20, 22, 23)):
         N = 1 << logn
         df = 0.1 / N
         freqs = (1.0 + np.arange(N, dtype=np.float64)) * df           # N bins ending at 0.1 Hz
@@ -226,7 +287,7 @@ def run_dense_sweep(args):
         M.mbhl_free(ctx0)
         ctx = M.mbhl_init(f_d, torch.as_tensor(data, device=dev), psd_d, sparse_points=S, max_batch=4096, device=local)
         M.mbhl_enable_stage_timing(ctx, True)
-        for B in (1, 16, 256, 1024, 4096):
+        for B in ((args.batch,) if args.batch else (1, 16, 256, 1024, 4096)):
             p = all_params[:B].copy()
             p[:, 10] *= scale_t
             params = torch.as_tensor(p, device=dev)
@@ -245,7 +306,7 @@ def run_dense_sweep(args):
             ms = e0.elapsed_time(e1) / steps
             stage = M.mbhl_stage_times(ctx)
             pairs, bins = M.mbhl_last_work(ctx)
-            flops = (FLOP_PER_PAIR * pairs + FLOP_PER_BIN * bins) * min(1.0, EXECUTED_OVER_TABLE_FLOPS)
+            flops, flops_table, flops_exec = dense_numerator(pairs, bins, M.mbhl_last_dense_work(ctx))
             fp64_ms = flops / (fp64_peak * 1e12) * 1e3
             hbm_ms = (80.0 * N * max(1, (B + 7) // 8) + B * 6 * (S - 1) * 256) / (hbm * 1e9) * 1e3
             print(json.dumps({"metric": METRIC, "value": B / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1, "steps": steps, "ms_per_step": ms,
@@ -255,7 +316,7 @@ def run_dense_sweep(args):
                                          "stage_ms": {k: float(v) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
                               "roofline": {"bound": "alu" if fp64_ms >= hbm_ms else "hbm", "dense_fp64_bound_ms": fp64_ms, "dense_hbm_bound_ms": hbm_ms,
                                            "frac": max(fp64_ms, hbm_ms) / stage[3], "frac_of_step": max(fp64_ms, hbm_ms) / ms,
-                                           "fp64_peak_tflops": fp64_peak},
+                                           "flops_table": flops_table, "flops_executed": flops_exec, "fp64_peak_tflops": fp64_peak},
                               "finite": bool(torch.isfinite(logL).all().item())}), flush=True)
         M.mbhl_free(ctx)
 
@@ -317,16 +378,27 @@ def run_sampler(args):
 
 
 def run_ours(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cpu = None
+    if args.cpu_baseline and rank == 0 and world == 1:
+        # the oracle over all host cores on a bounded sample, BEFORE this process touches CUDA (the workers are forked)
+        pool = OraclePool(args.config)
+        idx = pool.sample(16 if args.config == 2 else 8)
+        tcpu, _ = pool.time(idx)
+        pool.close()
+        cpu = {"value": len(idx) / tcpu, "unit": "logL/s", "cores": pool.cores, "kind": "oracle",
+               "sample": f"{len(idx)} walkers {idx} of the batch (spread over the injection groups), full grid, one walker per process, {tcpu:.1f} s"}
+
     import torch
     import torch.distributed as dist
 
     from paper_2005_01827_b200 import binding as M
     from paper_2005_01827_b200 import build as mbuild
+    from paper_2005_01827_b200 import shard
     from paper_2005_01827_b200 import workloads as W
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -338,6 +410,7 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     M.lib()
+    strong = args.scaling == "strong" and world > 1
 
     # ---- workload: grid, PSD, parameters from the seeded generators; injections from the library's own template ----
     state = {}
@@ -355,7 +428,7 @@ def run_ours(args):
     M.mbhl_free(state.pop("ctx0"))
     B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
     params_np = wl["params"]
-    if rank > 0:   # each rank gets its own walkers around the same injections (weak scaling)
+    if rank > 0 and not strong:   # weak scaling: each rank gets its own walkers around the same injections
         rng = np.random.default_rng(W.SEED0 + 1000 + rank)
         params_np = params_np * (1.0 + 1e-4 * rng.standard_normal(params_np.shape) * (np.arange(11) == 0))
     t = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=dev)
@@ -364,6 +437,23 @@ def run_ours(args):
     logL = torch.empty(B, dtype=torch.float64, device=dev)
     params_pin = torch.from_numpy(params_np.copy()).pin_memory()
     logL_pin = torch.empty(B, dtype=torch.float64).pin_memory()
+    if strong:
+        # strong scaling: ONE batch of B walkers, rows sharded across the ranks by the product's own sharding
+        # (paper_2005_01827_b200/shard.py: contiguous row ranges, all_gather of the logL slices over NCCL)
+        lo, hi = shard.shard_rows(B, world, rank)
+
+        def step():
+            out = shard.sharded_loglike(lambda rows: M.mbhl_loglike(ctx, rows), params)
+            logL.copy_(out)
+
+        def step_host():
+            M.mbhl_loglike_host(ctx, params_pin[lo:hi], logL_pin[lo:hi])
+    else:
+        def step():
+            M.mbhl_loglike(ctx, params, logL)
+
+        def step_host():
+            M.mbhl_loglike_host(ctx, params_pin, logL_pin)     # synchronous: returns after the D2H copy landed
 
     def barrier():
         if world > 1:
@@ -380,7 +470,7 @@ def run_ours(args):
     # ---- device-resident timing ----
     M.mbhl_enable_stage_timing(ctx, True)
     for _ in range(max(args.warmup, 3)):
-        M.mbhl_loglike(ctx, params, logL)
+        step()
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -390,23 +480,27 @@ def run_ours(args):
     barrier()
     e0.record()
     for _ in range(args.steps):
-        M.mbhl_loglike(ctx, params, logL)
+        step()
     e1.record()
     barrier()
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     launches = M.mbhl_launch_count(ctx) - launches0
     stage = np.array(M.mbhl_stage_times(ctx)) * args.steps       # mean over the timed steps (CUDA events on the launch stream)
     pairs, bins = M.mbhl_last_work(ctx)
+    counts = M.mbhl_last_dense_work(ctx)
     # ---- end to end: host buffers, H2D + D2H inside the timed region ----
-    M.mbhl_loglike_host(ctx, params_pin, logL_pin)
+    step_host()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        M.mbhl_loglike_host(ctx, params_pin, logL_pin)     # synchronous: returns after the D2H copy landed
+        step_host()
     torch.cuda.synchronize()
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     clocks = sampler.stop()
-    assert np.array_equal(logL_pin.numpy(), logL.cpu().numpy())
+    if strong:
+        assert np.array_equal(logL_pin.numpy()[lo:hi], logL.cpu().numpy()[lo:hi])
+    else:
+        assert np.array_equal(logL_pin.numpy(), logL.cpu().numpy())
 
     # ---- FP64 roofline denominator: DFMA-chain probe timed alone, in this run ----
     sink = torch.zeros(8, dtype=torch.float64, device=dev)
@@ -425,9 +519,11 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     ms_step = ms_total / args.steps
-    value = world * B * args.steps / (ms_total * 1e-3)
+    n_job = B if strong else world * B                      # walkers the whole job evaluates per step
+    n_rank = (hi - lo) if strong else B
+    value = n_job * args.steps / (ms_total * 1e-3)
     dense_ms = stage[3] / args.steps
-    flops = (FLOP_PER_PAIR * pairs + FLOP_PER_BIN * bins) * min(1.0, EXECUTED_OVER_TABLE_FLOPS)
+    flops, flops_table, flops_exec = dense_numerator(pairs, bins, counts)
     achieved = flops / (dense_ms * 1e-3) / 1e12
     peaks = {}
     try:
@@ -435,35 +531,49 @@ def run_ours(args):
     except OSError:
         pass
     hbm_bytes = 80.0 * bins          # weighted data + weights + frequency, if nothing were reused across walkers
+    traffic, traffic_src = DENSE_TRAFFIC.get(args.config, (None, None)) if not strong else (None, None)
     out = {
         "metric": METRIC, "value": value, "unit": "logL/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": workload_name(args.config, B, N, S), "walkers_per_gpu": B,
+        "config": {"workload": workload_name(args.config, B, N, S), "walkers_per_gpu": n_rank,
+                   "sharding": ("one batch, rows sharded by shard.sharded_loglike (all_gather of logL over NCCL)" if strong
+                                else "every rank its own batch, data replicated, no data-path collective"),
                    "l2": "inputs larger than L2 (0.34 GB weighted data + 1.6 GB spline coefficients per step vs 126 MB L2)",
                    "active_pairs_per_step": pairs, "active_bins_per_step": bins,
                    "stage_ms": {k: float(v / args.steps) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
-        "e2e": {"value": world * B * args.steps / e2e_s, "unit": "logL/s", "h2d_bytes_per_step": int(B * 11 * 8),
-                "d2h_bytes_per_step": int(B * 8)},
+        "e2e": {"value": n_job * args.steps / e2e_s, "unit": "logL/s", "h2d_bytes_per_step": int(n_rank * 11 * 8),
+                "d2h_bytes_per_step": int(n_rank * 8)},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": "k_dense", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                      "frac": achieved / fp64_peak, "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_of_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                     # dram__bytes_read.sum + dram__bytes_write.sum of one k_dense launch, from the committed ncu --set full capture
-                     "traffic": 2.04e9 if args.config == 2 else None, "traffic_source": "profiles/r01_dense_c2_final_ncu.txt (bytes per launch)",
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": "DFMA-chain probe measured in this run (nominal 148 SM x 64 lanes x 2 x 1.965 GHz = %.1f)" % NOMINAL_FP64_TFLOPS,
-                     "algorithmic_flops_per_launch": flops, "dense_ms": dense_ms,
+                     "algorithmic_flops_per_launch": flops, "flops_table": flops_table, "flops_executed": flops_exec,
+                     "numerator": "lesser of the SURVEY 8(d) table count and the count executed (k_dense's own tallies, this run)",
+                     "dense_ms": dense_ms,
                      "hbm_bound_ms_if_no_reuse": hbm_bytes / (peaks.get("hbm_gbs", 6650.0) * 1e9) * 1e3},
     }
-    if args.cpu_baseline:
-        table, owl, idx = oracle_sample(args.config)
-        tcpu = time_oracle(table, owl, idx)
-        out["cpu_baseline"] = {"value": len(idx) / tcpu, "unit": "logL/s", "cores": 1, "kind": "oracle",
-                               "sample": f"walkers {idx} of the batch (one per injection group), full grid, {tcpu:.1f} s"}
+    if cpu is not None:
+        out["cpu_baseline"] = cpu
     print(json.dumps(out))
     M.mbhl_free(ctx)
     if world > 1:
         dist.destroy_process_group()
+
+
+def spawn_ranks(args):
+    """python bench.py --gpus N without a launcher: re-run this file under torch.distributed.run, one rank per GPU."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd, env=env))
 
 
 def main():
@@ -475,8 +585,11 @@ def main():
                     help="BASELINE.json config; 0-2 are likelihood workloads (2 = default bench line), 3 = sparse-stage isolation, "
                          "4 = dense N x B sweep (one JSON line per point)")
     ap.add_argument("--sampler", action="store_true", help="time the parallel-tempered stretch-move ensemble (SURVEY 8(f).2) on the config-2 data")
-    ap.add_argument("--batch", type=int, default=0, help="config 3 only: number of parameter sets (default 16384)")
+    ap.add_argument("--batch", type=int, default=0, help="config 3: number of parameter sets (default 16384); config 4: only this batch size")
+    ap.add_argument("--logn", type=int, default=0, help="config 4: only the grid with N = 2^logn bins")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--scaling", default="weak", choices=("weak", "strong"),
+                    help="N > 1: weak = every rank its own batch of B walkers; strong = ONE batch sharded across the ranks (shard.py)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -490,8 +603,8 @@ def main():
     elif args.config == 4:
         run_dense_sweep(args)
     else:
-        if int(os.environ.get("WORLD_SIZE", "1")) > 1 or args.gpus > 1:
-            args.cpu_baseline = args.cpu_baseline and int(os.environ.get("RANK", "0")) == 0 and int(os.environ.get("WORLD_SIZE", "1")) == 1
+        if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            spawn_ranks(args)
         run_ours(args)
 
 

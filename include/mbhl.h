@@ -178,6 +178,14 @@ int64_t mbhl_launch_count(const mbhl_ctx* ctx);     /* kernels this context has 
  * pairs = sum over walkers and modes of in-band bins, bins = sum over walkers of bins covered by >= 1 mode. */
 int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins);
 
+/* What the fused dense kernel EXECUTED in the last mbhl_loglike* call (counted in the kernel, one tally per warp), for
+ * the roofline numerator: counts[0] calls of the uniform-record evaluator, counts[1] of its gated form, counts[2] of the
+ * per-bin-record evaluator - each call evaluates one mode at 4 bins on all 32 lanes of a warp, in band or not -,
+ * counts[3] single (lane, bin, mode) evaluations of the global per-bin path, counts[4] inner-product epilogues (each
+ * covers one walker at the 128 bins of a warp).  With slices (B > 32768) the counts are those of the last slice.
+ * Synchronises the stream.                                                                                          */
+int mbhl_last_dense_work(mbhl_ctx* ctx, int64_t counts[5]);
+
 /* Optional per-stage device timing.  When enabled, mbhl_loglike* records CUDA events on the context's stream
  * around its five stages; mbhl_stage_times synchronises the stream, returns the MEAN milliseconds per stage
  * over the calls made since the previous mbhl_stage_times / enable (at most the last 64) and resets the

@@ -17,7 +17,7 @@ COORDS_PHYSICAL, COORDS_SAMPLED, COORDS_SAMPLED_LISA = 0, 1, 2        # include/
 SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
            "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
-           "mbhl_launch_count", "mbhl_last_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
+           "mbhl_launch_count", "mbhl_last_work", "mbhl_last_dense_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
 
 
 class mbhl_config(ctypes.Structure):
@@ -68,6 +68,7 @@ def lib():
         L.mbhl_launch_count.argtypes = [vp]
         L.mbhl_launch_count.restype = i64
         L.mbhl_last_work.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        L.mbhl_last_dense_work.argtypes = [vp, ctypes.POINTER(i64 * 5)]
         L.mbhl_enable_stage_timing.argtypes = [vp, i32]
         L.mbhl_stage_times.argtypes = [vp, ctypes.POINTER(dbl * 5)]
         L.mbhl_dfma_probe.argtypes = [vp, i32, i32, i64, vp]
@@ -186,6 +187,13 @@ def mbhl_last_work(ctx):
     p, b = ctypes.c_int64(), ctypes.c_int64()
     _check(lib().mbhl_last_work(ctx, ctypes.byref(p), ctypes.byref(b)), ctx)
     return p.value, b.value
+
+
+def mbhl_last_dense_work(ctx):
+    """(uniform calls, gated calls, per-bin-record calls, single lane evaluations, epilogues) of the last dense launch."""
+    c = (ctypes.c_int64 * 5)()
+    _check(lib().mbhl_last_dense_work(ctx, ctypes.byref(c)), ctx)
+    return tuple(int(v) for v in c)
 
 
 def mbhl_enable_stage_timing(ctx, on=True):

@@ -212,7 +212,8 @@ int run_dense(mbhl_ctx* ctx, int64_t B, char* base, const WsLayout& L, uint32_t 
     A.n_groups = P.n_groups;
     A.inv_df = 1.0 / ctx->df;
     A.mode_mask = mode_mask;
-    if (count_work) CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    if (count_work) CU(cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), ctx->stream));
+    A.work = count_work ? ctx->counters + 2 : nullptr;
     const bool tm = ctx->timing && count_work;
     if (tm) cudaEventRecord(ctx->ev[3], ctx->stream);
     k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);
@@ -304,7 +305,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     const int nblk = (int)((N + 1023) / 1024) > n_chunks_of(N) ? (int)((N + 1023) / 1024) : n_chunks_of(N);
     if (cudaMalloc(&ctx->freqs, nb) != cudaSuccess ||
         cudaMalloc(&ctx->tiles, (size_t)n_chunks_of(N) * kTileBytes) != cudaSuccess ||
-        cudaMalloc(&ctx->counters, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMalloc(&ctx->counters, 8 * sizeof(unsigned long long)) != cudaSuccess ||
         cudaMalloc(&d_part, (size_t)nblk * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
         return cleanup(MBHL_ENOMEM);
@@ -347,7 +348,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
     host_part.resize(nch);
     k_init_tiles<<<nch, 256, 0, st>>>(ctx->freqs, data_dev, psd_dev, N, ctx->df, ctx->tiles, d_part);
     if (cudaMemcpyAsync(host_part.data(), d_part, (size_t)nch * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-        cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess ||
+        cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
     ctx->launches += 2;
@@ -623,6 +624,15 @@ int mbhl_last_work(mbhl_ctx* ctx, int64_t* pairs, int64_t* bins) {
     CU(cudaStreamSynchronize(ctx->stream));
     if (pairs) *pairs = (int64_t)h[0];
     if (bins) *bins = (int64_t)h[1];
+    return MBHL_OK;
+}
+
+int mbhl_last_dense_work(mbhl_ctx* ctx, int64_t counts[5]) {
+    if (!ctx || !counts) return MBHL_EINVAL;
+    unsigned long long h[8];
+    CU(cudaMemcpyAsync(h, ctx->counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < 5; ++i) counts[i] = (int64_t)h[2 + i];
     return MBHL_OK;
 }
 

@@ -254,6 +254,9 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
 
     const uint32_t bar = smem_u32(&s_bar);
     uint32_t parity = 0;
+    // executed-work tallies of this warp (warp-uniform; mbhl_last_dense_work): calls of the uniform / gated / per-bin-record
+    // evaluators (each evaluates kDenseR bins on all 32 lanes), lane evaluations of the global per-bin path, epilogues
+    unsigned n_uni = 0, n_gat = 0, n_rec = 0, n_lane = 0, n_epi = 0;
     for (int chunk = c_first; chunk <= c_last; ++chunk) {
         __syncthreads();                                            // every reader of the previous tile / records is done
         if (tid == 0) {
@@ -354,6 +357,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                 m_full &= m_full - 1;
                 const int slot = 2 * (wi * MBHL_NMODE + mi) + ((m_selB >> mi) & 1u);
                 mode_uniform<false>(s_rec + slot * kCoefStride, s_xj[slot], f, f, h);
+                ++n_uni;
             }
             while (m_part) {
                                 const int mi = __ffs(m_part) - 1;
@@ -375,6 +379,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                         gate[r] = (o >= lo0 && o <= hi1) ? 1.0 : 0.0;
                     }
                     mode_perbin(rec, u, gate, h);
+                    ++n_rec;
                 } else {
                     // band edge: the one staged segment is evaluated on all bins with the amplitude gated
                     const int seg = (lo1 <= hi1) ? 1 : 0;
@@ -386,6 +391,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                         gate[r] = (o >= lo && o <= hi) ? 1.0 : 0.0;
                     }
                     mode_uniform<true>(s_rec + (slot0 + seg) * kCoefStride, s_xj[slot0 + seg], f, gate, h);
+                    ++n_gat;
                 }
             }
             if (m_gen) {
@@ -412,6 +418,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                     const double* cbase = A.coef + ((int64_t)(b0 + wi) * MBHL_NMODE + mi) * (int64_t)(A.S - 1) * kCoefStride;
                     if (ja_m == jb_m && full_m) {
                         mode_uniform<false>(cbase + (int64_t)ja_m * kCoefStride, __ldg(x + ja_m), f, f, h);
+                        ++n_uni;
                     } else if (jb_m - ja_m < kGenSlots) {
                         // a few intervals in the warp tile: their records and knots are copied to this warp's scratch with
                         // independent loads (one L2 round trip), then every bin looks its interval up in shared memory
@@ -436,11 +443,13 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                             gate[r] = (k >= k_lo && k <= k_hi) ? 1.0 : 0.0;
                         }
                         mode_perbin(rec, u, gate, h);
+                        ++n_rec;
                     } else {
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
 #pragma unroll
                         for (int r = 0; r < kDenseR; ++r) {
                             const int k = kt0 + lane + 32 * r;
+                            n_lane += __popc(__ballot_sync(0xffffffffu, k >= k_lo && k <= k_hi));
                             if (k < k_lo || k > k_hi) continue;
                             int j = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
                             while (j > ja_m && f[r] < __ldg(x + j)) --j;
@@ -483,7 +492,15 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
 #pragma unroll
             for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if ((lane & 15) == 0) s_acc[warp][wi][lane >> 4] += v;
+            ++n_epi;
         }
+    }
+    if (A.work != nullptr && lane == 0) {
+        if (n_uni) atomicAdd(A.work + 0, (unsigned long long)n_uni);
+        if (n_gat) atomicAdd(A.work + 1, (unsigned long long)n_gat);
+        if (n_rec) atomicAdd(A.work + 2, (unsigned long long)n_rec);
+        if (n_lane) atomicAdd(A.work + 3, (unsigned long long)n_lane);
+        if (n_epi) atomicAdd(A.work + 4, (unsigned long long)n_epi);
     }
     __syncthreads();
     if (tid < nb) {

@@ -452,6 +452,7 @@ struct DenseArgs {
     int n_groups;
     double inv_df;           // 1 / bin spacing of the init grid
     uint32_t mode_mask;      // modes evaluated by this launch (bit i = mode i); the others count as out of band
+    unsigned long long* work; // [5] executed-work tallies (may be null): see mbhl_last_dense_work
 };
 
 // sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
