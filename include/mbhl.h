@@ -189,9 +189,9 @@ int mbhl_last_dense_work(mbhl_ctx* ctx, int64_t counts[5]);
 /* Optional per-stage device timing.  When enabled, mbhl_loglike* records CUDA events on the context's stream
  * around its five stages; mbhl_stage_times synchronises the stream, returns the MEAN milliseconds per stage
  * over the calls made since the previous mbhl_stage_times / enable (at most the last 64) and resets the
- * count: ms[0] per-walker constants, ms[1] sparse evaluation, ms[2] spline solve, ms[3] fused dense kernel,
- * ms[4] final reduction (mbhl_sparse is timed too, with ms[3] = ms[4] = 0).  Returns MBHL_EINVAL if timing
- * is off or no call was made.                                                                            */
+ * count: ms[0] per-walker constants, ms[1] the fused sparse kernel (PhenomHM + response at the knots + spline
+ * coefficients), ms[2] = 0 (kept for layout), ms[3] fused dense kernel, ms[4] final reduction (mbhl_sparse is timed too,
+ * with ms[3] = ms[4] = 0).  Returns MBHL_EINVAL if timing is off or no call was made.                        */
 int mbhl_enable_stage_timing(mbhl_ctx* ctx, int32_t on);
 int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]);
 

@@ -44,7 +44,7 @@ namespace {
 constexpr int64_t kSliceBatch = 32768;   // walkers per pass of the hot path; larger batches are processed in slices
 
 struct WsLayout {
-    size_t params, consts, dense, knots, y, coef, partials, dh, hh, logl, total;
+    size_t params, consts, dense, knots, coef, partials, dh, hh, logl, total;
 };
 
 // Launch shape of the fused dense kernel: W walkers per CTA tile, G chunks per CTA.  W amortises the staged
@@ -89,7 +89,6 @@ WsLayout layout(const mbhl_ctx* c, int64_t B) {
     L.consts = off; off += align256(b * sizeof(WalkerConst));
     L.dense = off; off += align256(b * sizeof(DenseWalker));
     L.knots = off; off += align256(b * MBHL_NMODE * c->S * sizeof(double));
-    L.y = off; off += align256(b * MBHL_NMODE * MBHL_NQ * c->S * sizeof(double));
     L.coef = off; off += align256(b * MBHL_NMODE * (size_t)(c->S - 1) * kCoefStride * sizeof(double));
     L.partials = off; off += align256(partials_capacity(b, n_chunks_of(c->N)) * 2 * sizeof(double));
     L.dh = off; off += align256(b * sizeof(double));
@@ -147,14 +146,14 @@ bool is_device_ptr(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-// k_spline's dynamic shared memory limit is per function and per device, not per context: keep the running maximum
-// so that contexts with different S can coexist (several contexts may be alive at once, mbhl.h).
+// The fused sparse kernel's dynamic shared memory limit is per function and per device, not per context: keep the
+// running maximum so that contexts with different S can coexist (several contexts may be alive at once, mbhl.h).
 int ensure_spline_smem(mbhl_ctx* ctx) {
     static size_t granted[64] = {0};
     const size_t need = spline_smem_bytes(ctx->S);
     const int d = ctx->device & 63;
     if (granted[d] < need) {
-        CU(cudaFuncSetAttribute(k_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+        CU(cudaFuncSetAttribute(k_sparse_spline, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
         granted[d] = need;
     }
     return MBHL_OK;
@@ -168,28 +167,24 @@ void run_consts(mbhl_ctx* ctx, const double* rows_dev, int64_t B, int coords, ch
     ctx->launches += 1;
 }
 
-// Runs the sparse stage (a1-a5) for rows already on the device.
-int run_sparse(mbhl_ctx* ctx, const double* rows_dev, int64_t B, int coords, char* base, const WsLayout& L, bool with_coef) {
-    WalkerConst* wc = (WalkerConst*)(base + L.consts);
-    double* knots = (double*)(base + L.knots);
-    double* y = (double*)(base + L.y);
-    double* coef = (double*)(base + L.coef);
+// Runs the sparse stage (a1-a5) for rows already on the device: the per-walker constants, then (with_coef) the fused
+// PhenomHM + response + spline kernel, one cluster of two CTAs per (walker, mode).  y_out: optional export of the knot values.
+int run_sparse(mbhl_ctx* ctx, const double* rows_dev, int64_t B, int coords, char* base, const WsLayout& L, bool with_coef,
+               double* y_out = nullptr) {
     const int S = ctx->S;
     const bool tm = ctx->timing && with_coef;
     if (tm) ctx->ev = ctx->evs[ctx->n_timed % mbhl_ctx::kSlots];
     if (tm) cudaEventRecord(ctx->ev[0], ctx->stream);
     run_consts(ctx, rows_dev, B, coords, base, L);
     if (tm) cudaEventRecord(ctx->ev[1], ctx->stream);
-    dim3 gs((unsigned)(B * MBHL_NMODE), (unsigned)((S + 127) / 128));
-    k_sparse_eval<<<gs, 128, 0, ctx->stream>>>(wc, S, knots, y);
-    ctx->launches += 1;
-    if (tm) cudaEventRecord(ctx->ev[2], ctx->stream);
     if (with_coef) {
         int rc = ensure_spline_smem(ctx);
         if (rc != MBHL_OK) return rc;
-        k_spline<<<(unsigned)(B * MBHL_NMODE * 2), kSplineThreads, spline_smem_bytes(S), ctx->stream>>>(wc, S, knots, y, coef);
+        k_sparse_spline<<<(unsigned)(B * MBHL_NMODE * 2), kSplineThreads, spline_smem_bytes(S), ctx->stream>>>(
+            (const WalkerConst*)(base + L.consts), S, (double*)(base + L.knots), (double*)(base + L.coef), y_out);
         ctx->launches += 1;
     }
+    if (tm) { cudaEventRecord(ctx->ev[2], ctx->stream); cudaEventRecord(ctx->ev[3], ctx->stream); }
     CU(cudaGetLastError());
     return MBHL_OK;
 }
@@ -296,7 +291,7 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         if (cudaMemcpyToSymbol(c_prior_lo, lo, sizeof(lo)) != cudaSuccess || cudaMemcpyToSymbol(c_prior_hi, hi, sizeof(hi)) != cudaSuccess)
             return cleanup(MBHL_ECUDA);
     }
-    if (cudaFuncSetAttribute(k_spline, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
+    if (cudaFuncSetAttribute(k_sparse_spline, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
         cudaFuncSetAttribute(k_dense, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess)
         return cleanup(MBHL_ECUDA);
     if (cudaFuncSetAttribute(k_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, kDenseSmemBytes) != cudaSuccess)
@@ -670,7 +665,7 @@ int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, d
     int rc = get_workspace(ctx, B, &base);
     if (rc != MBHL_OK) return rc;
     const WsLayout L = layout(ctx, B);
-    rc = run_sparse(ctx, params, B, MBHL_COORDS_PHYSICAL, base, L, true);
+    rc = run_sparse(ctx, params, B, MBHL_COORDS_PHYSICAL, base, L, true, y);      // y lands in the caller's buffer, phase row in cycles
     if (rc != MBHL_OK) return rc;
     if (ctx->timing) {   // stages 3 and 4 (dense, reduce) do not run here: zero-length intervals
         for (int i = 3; i < 6; ++i) cudaEventRecord(ctx->ev[i], ctx->stream);
@@ -680,7 +675,7 @@ int mbhl_sparse(mbhl_ctx* ctx, const double* params, int64_t B, double* knots, d
     if (knots) CU(cudaMemcpyAsync(knots, base + L.knots, nk * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     if (y) {
         const int64_t rows = B * MBHL_NMODE * MBHL_NQ;
-        k_export_y<<<(unsigned)((rows * ctx->S + 255) / 256), 256, 0, ctx->stream>>>((const double*)(base + L.y), rows, ctx->S, y);
+        k_export_y<<<(unsigned)((rows * ctx->S + 255) / 256), 256, 0, ctx->stream>>>(y, rows, ctx->S, y);   // in place: phase row to radians
         ctx->launches += 1;
     }
     if (coef) {

@@ -194,53 +194,7 @@ __global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const doubl
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3 + a4: PhenomHM + response at the sparse knots, one thread per (walker, mode, knot)
-// y layout [walker][mode][q][S], phase row in cycles; knots [walker][mode][S]
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_sparse_eval(const WalkerConst* __restrict__ wc, int S, double* __restrict__ knots,
-                                                     double* __restrict__ y) {
-    const int64_t bm = blockIdx.x;                  // walker * 6 + mode
-    const int64_t b = bm / MBHL_NMODE;
-    const int mi = (int)(bm - b * MBHL_NMODE);
-    const int s = blockIdx.y * blockDim.x + threadIdx.x;
-    // the CTA's 128 knots belong to one (walker, mode): its constants are read from shared memory
-    __shared__ WalkerConst s_c;
-    for (int i = threadIdx.x; i < (int)(sizeof(WalkerConst) / 8); i += blockDim.x)
-        reinterpret_cast<double*>(&s_c)[i] = reinterpret_cast<const double*>(wc + b)[i];
-    __syncthreads();
-    if (s >= S) return;
-    const WalkerConst& c = s_c;
-    double q[MBHL_NQ];
-    double f = 0.0;
-    if (c.valid && c.mode[mi].active) {
-        const ModeConst& mc = c.mode[mi];
-        f = (s == 0) ? mc.f_lo : ((s == S - 1) ? mc.f_hi : mc.f_lo * exp(s * mc.dlog));
-        smooth_quantities(c, mi, f, q);
-    } else {
-#pragma unroll
-        for (int i = 0; i < MBHL_NQ; ++i) q[i] = 0.0;
-    }
-    knots[bm * S + s] = f;
-#pragma unroll
-    for (int i = 0; i < MBHL_NQ; ++i) y[(bm * MBHL_NQ + i) * S + s] = q[i];
-}
-
-// ---------------------------------------------------------------------------------------------
-// a5: not-a-knot cubic spline coefficients.  The slope system of one
-// (walker, mode) is tridiagonal, strictly diagonally dominant and shared by the 8 splined quantities.  One
-// CTA of 4 warps handles (walker, mode, half) with half = quantities 0-3 or 4-7, so two CTAs fit in one
-// SM's shared memory at S = 1024.  Every recurrence of the Thomas algorithm is contractive here (factors
-// 0.07 for the pivots, 0.27 for both sweeps on log-spaced knots), so each is cut into blocks that start a
-// few rows early from a zero state ("halo"): the influence of the cut is below fp64 rounding after 16
-// (pivots) / 32 (sweeps) rows, and blocks that reach row 0 / S-1 use the true not-a-knot rows.
-//   A. 1/h_r; pivots: thread t owns ceil(S/128) rows: c'_r = u_r / (d_r - a_r c'_{r-1}), 1 division per row
-//   B. b_r = rhs_r / (d_r - a_r c'_{r-1}) for 4 quantities, all rows in parallel
-//   C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows)
-//   D. backward sweep s_r = g_r - c'_r s_{r+1}
-//   E. c_j, d_j of every interval; records written as 128-byte half records
-// coef layout [walker][mode][interval][q][4] = (y_j, s_j, c_j, d_j).  Phase row (q = 1) as the dense kernel wants it:
-// quarter turns, linear term folded in: 4 [(y_j mod 1) - frac(x_j t_coal)], 4 (s_j - t_coal), 4 c_j, 4 d_j, so that
-// the total phase of a bin is ONE cubic in u = f - x_j (mbhl_sparse converts back to cycles on export).
+// a3 + a4 + a5: the fused sparse stage (PhenomHM + response at the knots, spline coefficients): mbhl_sparse.cuh
 // ---------------------------------------------------------------------------------------------
 constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
 
@@ -252,185 +206,11 @@ __device__ __forceinline__ double linear_cycles(double f, double t) {
     return (p - pr) + e;
 }
 
-__device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
+}  // namespace mbhl
 
-constexpr int kSplineQ = 4;              // quantities per CTA
-constexpr int kSplineThreads = 256;      // 8 warps for the row-parallel phases; warps 0-3 run the sweeps (one quantity each)
-constexpr int kSplineHaloPivot = 16;
-constexpr int kSplineHaloSweep = 32;
+#include "mbhl_sparse.cuh"
 
-// Row strides (in doubles) congruent to 4 mod 16: the last phase reads rows q = 0..3 at intervals j..j+3 from one
-// half-warp, and 4 q + j then covers the 16 bank pairs once (a stride of S or S + S/32 + 1 gives 4-way conflicts).
-__host__ __device__ inline int spline_stride(int n) { return n + ((4 - n % 16) + 16) % 16; }
-__host__ __device__ inline int spline_sp(int S) { return spline_stride(S + (S >> 5) + 1); }
-
-__host__ __device__ inline size_t spline_smem_bytes(int S) {
-    return (size_t)(5 + kSplineQ) * spline_sp(S) * sizeof(double) + (size_t)kSplineQ * spline_stride(S) * sizeof(double);
-}
-
-__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src)
-                 : "memory");
-}
-
-__global__ void __launch_bounds__(kSplineThreads) k_spline(const WalkerConst* __restrict__ wc, int S, const double* __restrict__ knots,
-                                                const double* __restrict__ y, double* __restrict__ coef) {
-    extern __shared__ double sm[];
-    const int SP = spline_sp(S), SY = spline_stride(S);
-    double* xk = sm;                     // knots                                  [SP]
-    double* ih = xk + SP;                // 1 / h_r, h_r = x_{r+1} - x_r          [SP]
-    double* cps = ih + SP;               // pivots c'_r                            [SP]
-    double* ivs = cps + SP;              // 1 / (d_r - a_r c'_{r-1})               [SP]
-    double* mls = ivs + SP;              // a_r / (d_r - a_r c'_{r-1})             [SP]
-    double* A1 = mls + SP;               // b, then g, then the slopes s (in place) [4][SP]
-    double* Y = A1 + kSplineQ * SP;      // y values of the 4 quantities           [4][SY]
-    const int64_t bm = blockIdx.x >> 1;
-    const int half = blockIdx.x & 1;
-    const int64_t b = bm / MBHL_NMODE;
-    const int mi = (int)(bm - b * MBHL_NMODE);
-    const int tid = threadIdx.x;
-    double* cout = coef + bm * (int64_t)(S - 1) * kCoefStride + half * (kSplineQ * 4);
-    const bool active = wc[b].valid && wc[b].mode[mi].active;
-    const double t_coal = wc[b].t_coal;
-    if (!active) {
-        for (int idx = tid; idx < (S - 1) * kSplineQ * 2; idx += blockDim.x) {
-            const int j = idx >> 3, i = idx & 7;
-            reinterpret_cast<double2*>(cout + (int64_t)j * kCoefStride)[i] = make_double2(0.0, 0.0);
-        }
-        return;
-    }
-    // all global reads of this CTA are issued up front as asynchronous copies: knots (group 0), y (group 1)
-    const double* xg = knots + bm * S;
-    const double* yg = y + (bm * MBHL_NQ + half * kSplineQ) * S;
-    for (int i = tid; i < S; i += blockDim.x) cp_async8(xk + pad_idx(i), xg + i);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    for (int i = tid; i < kSplineQ * S; i += blockDim.x) cp_async8(Y + (i / S) * SY + i % S, yg + i);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    asm volatile("cp.async.wait_group 1;" ::: "memory");
-    __syncthreads();
-    // matrix row r: (lower a, diag d, upper u)
-    auto mat = [&](int r, double& a, double& d, double& u) {
-        if (r == 0) {
-            const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
-            a = 0.0; d = h1; u = h0 + h1;
-        } else if (r == S - 1) {
-            const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
-            a = hm + hn; d = hn; u = 0.0;
-        } else {
-            const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
-            a = hr; d = 2.0 * (hl + hr); u = hl;
-        }
-    };
-    // A. reciprocal spacings and pivots
-    for (int r = tid; r < S - 1; r += blockDim.x) ih[pad_idx(r)] = 1.0 / (xk[pad_idx(r + 1)] - xk[pad_idx(r)]);
-    {
-        const int m = (S + (int)blockDim.x - 1) / (int)blockDim.x;
-        const int own0 = tid * m, own1 = min(S, own0 + m);
-        if (own0 < own1) {
-            double cp = 0.0;
-            for (int r = max(0, own0 - kSplineHaloPivot); r < own1; ++r) {
-                double a, d, u;
-                mat(r, a, d, u);
-                const double inv = 1.0 / (d - a * cp);
-                cp = u * inv;
-                if (r >= own0) { cps[pad_idx(r)] = cp; ivs[pad_idx(r)] = inv; mls[pad_idx(r)] = a * inv; }
-            }
-        }
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    __syncthreads();
-    // B. scaled right-hand sides of the slope system, all rows in parallel
-    for (int idx = tid; idx < kSplineQ * S; idx += blockDim.x) {
-        const int q = idx / S, r = idx - q * S;
-        const double* yq = Y + q * SY;
-        double v;
-        if (r == 0) {
-            const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
-            const double d0 = (yq[1] - yq[0]) * ih[pad_idx(0)], d1 = (yq[2] - yq[1]) * ih[pad_idx(1)];
-            v = ((3.0 * h0 + 2.0 * h1) * h1 * d0 + h0 * h0 * d1) / (h0 + h1);
-        } else if (r == S - 1) {
-            const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
-            const double dm = (yq[S - 1] - yq[S - 2]) * ih[pad_idx(S - 2)], dn = (yq[S - 2] - yq[S - 3]) * ih[pad_idx(S - 3)];
-            v = (hm * hm * dn + (2.0 * hn + 3.0 * hm) * hn * dm) / (hn + hm);
-        } else {
-            const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
-            const double yr = yq[r];
-            v = 3.0 * (hr * ((yr - yq[r - 1]) * ih[pad_idx(r - 1)]) + hl * ((yq[r + 1] - yr) * ih[pad_idx(r)]));
-        }
-        A1[q * SP + pad_idx(r)] = v * ivs[pad_idx(r)];
-    }
-    __syncthreads();
-    // C, D. sweeps in place: warp = quantity, lane = block of rows.  A lane first copies the halo rows it needs
-    // from its neighbour's block into registers, so the neighbour may overwrite them afterwards.
-    if (tid < 32 * kSplineQ) {
-        const int q = tid >> 5, lane = tid & 31;
-        const int m = (S + 31) / 32;
-        const int own0 = lane * m, own1 = min(S, own0 + m);
-        double* aq = A1 + q * SP;
-        double halo[kSplineHaloSweep];
-#pragma unroll
-        for (int i = 0; i < kSplineHaloSweep; ++i) {
-            const int r = own0 - kSplineHaloSweep + i;
-            halo[i] = (r >= 0 && r < S) ? aq[pad_idx(r)] : 0.0;
-        }
-        __syncwarp();
-        if (own0 < own1) {
-            double g = 0.0;
-#pragma unroll
-            for (int i = 0; i < kSplineHaloSweep; ++i) {
-                const int r = own0 - kSplineHaloSweep + i;
-                if (r >= 0) g = fma(-mls[pad_idx(r)], g, halo[i]);
-            }
-            for (int r = own0; r < own1; ++r) {
-                g = fma(-mls[pad_idx(r)], g, aq[pad_idx(r)]);
-                aq[pad_idx(r)] = g;
-            }
-        }
-        __syncwarp();
-#pragma unroll
-        for (int i = 0; i < kSplineHaloSweep; ++i) {
-            const int r = own1 + i;
-            halo[i] = (r < S) ? aq[pad_idx(r)] : 0.0;
-        }
-        __syncwarp();
-        if (own0 < own1) {
-            double sl = 0.0;
-#pragma unroll
-            for (int i = kSplineHaloSweep - 1; i >= 0; --i) {
-                const int r = own1 + i;
-                if (r < S) sl = fma(-cps[pad_idx(r)], sl, halo[i]);
-            }
-            for (int r = own1 - 1; r >= own0; --r) {
-                sl = fma(-cps[pad_idx(r)], sl, aq[pad_idx(r)]);
-                aq[pad_idx(r)] = sl;
-            }
-        }
-    }
-    __syncthreads();
-    // E. coefficients: one (interval, quantity) per thread, 32 B each; 4 consecutive threads write a 128-byte half record
-    for (int idx = tid; idx < (S - 1) * kSplineQ; idx += blockDim.x) {
-        const int j = idx >> 2, q = idx & 3;
-        const double hinv = ih[pad_idx(j)];
-        double y0 = Y[q * SY + j];
-        const double y1 = Y[q * SY + j + 1];
-        const double s0 = A1[q * SP + pad_idx(j)], s1 = A1[q * SP + pad_idx(j + 1)];
-        const double dl = (y1 - y0) * hinv;
-        const double cc = (3.0 * dl - 2.0 * s0 - s1) * hinv;
-        const double dd = (s0 + s1 - 2.0 * dl) * (hinv * hinv);
-        double s0w = s0, ccw = cc, ddw = dd;
-        if (half == 0 && q == 1) {
-            // phase row: quarter turns, with the linear term -f t_coal of the total phase (reading G9) folded in.
-            // f t_coal = x_j t_coal + u t_coal: the first product is reduced mod 1 exactly, the second joins the slope.
-            y0 = 4.0 * ((y0 - rint(y0)) - linear_cycles(xk[pad_idx(j)], t_coal));
-            s0w = 4.0 * (s0 - t_coal);
-            ccw = 4.0 * cc;
-            ddw = 4.0 * dd;
-        }
-        double2* o = reinterpret_cast<double2*>(cout + (int64_t)j * kCoefStride + q * 4);
-        o[0] = make_double2(y0, s0w);
-        o[1] = make_double2(ccw, ddw);
-    }
-}
+namespace mbhl {
 
 // ---------------------------------------------------------------------------------------------
 // a6 + a7: fused dense kernel (mbhl_dense.cuh, which documents the work decomposition): interpolates every
@@ -613,7 +393,7 @@ __global__ void __launch_bounds__(128) k_template(const WalkerConst* __restrict_
 }
 
 // mbhl_sparse: copy of the y rows with the phase row converted to radians
-__global__ void k_export_y(const double* __restrict__ y, int64_t n_rows, int S, double* __restrict__ out) {
+__global__ void k_export_y(const double* y, int64_t n_rows, int S, double* out) {   // out may alias y
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_rows * S) return;
     const int64_t row = i / S;
