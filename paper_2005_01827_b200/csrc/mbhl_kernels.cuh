@@ -196,8 +196,6 @@ __global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const doubl
 // ---------------------------------------------------------------------------------------------
 // a3 + a4 + a5: the fused sparse stage (PhenomHM + response at the knots, spline coefficients): mbhl_sparse.cuh
 // ---------------------------------------------------------------------------------------------
-constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
-
 // frac(f * t) in cycles with the product taken exactly (reading G9): f and t are the supplied doubles.
 __device__ __forceinline__ double linear_cycles(double f, double t) {
     const double p = f * t;
@@ -234,49 +232,6 @@ struct DenseArgs {
     uint32_t mode_mask;      // modes evaluated by this launch (bit i = mode i); the others count as out of band
     unsigned long long* work; // [5] executed-work tallies (may be null): see mbhl_last_dense_work
 };
-
-// sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
-// (Chebyshev-node interpolation in 50-digit arithmetic; max error 2.6e-17 / 1.0e-16 before rounding).
-// Kept in the constant bank so that DFMA reads them as c[][] operands (as immediates each costs two moves per use).
-__constant__ double c_sc[13] = {1.5707963267948966, -0.6459640975062443, 0.07969262624604301, -0.004681754132340976,
-                                0.0001604411507421909, -3.59864335298231e-06, 5.633933781537854e-08,
-                                -1.2337005501361513, 0.25366950789986475, -0.02086348073494657,
-                                0.000919259950041661, -2.520013526428479e-05, 4.6552961874867623e-07};
-#define kS0 c_sc[0]
-#define kS1 c_sc[1]
-#define kS2 c_sc[2]
-#define kS3 c_sc[3]
-#define kS4 c_sc[4]
-#define kS5 c_sc[5]
-#define kS6 c_sc[6]
-#define kC1 c_sc[7]
-#define kC2 c_sc[8]
-#define kC3 c_sc[9]
-#define kC4 c_sc[10]
-#define kC5 c_sc[11]
-#define kC6 c_sc[12]
-
-// sin and cos of p4 quarter turns (angle = p4 pi/2), any |p4| < 2^51.  No conversions, no divides: the
-// nearest integer comes from the magic-number add, the quadrant from the low word of that sum.
-__device__ __forceinline__ void sincos_qturn(double p4, double& sn, double& cs) {
-    const double t = p4 + kRoundMagic;
-    const int n = __double2loint(t);
-    const double y = p4 - (t - kRoundMagic);
-    const double z = y * y;
-    double ps = fma(z, kS6, kS5);
-    double pc = fma(z, kC6, kC5);
-    ps = fma(z, ps, kS4); pc = fma(z, pc, kC4);
-    ps = fma(z, ps, kS3); pc = fma(z, pc, kC3);
-    ps = fma(z, ps, kS2); pc = fma(z, pc, kC2);
-    ps = fma(z, ps, kS1); pc = fma(z, pc, kC1);
-    ps = fma(z, ps, kS0); pc = fma(z, pc, 1.0);
-    ps *= y;
-    const bool odd = (n & 1) != 0;
-    const double a = odd ? pc : ps;      // sin(angle) up to sign
-    const double b = odd ? ps : pc;      // cos(angle) up to sign
-    sn = __hiloint2double(__double2hiint(a) ^ ((n & 2) << 30), __double2loint(a));
-    cs = __hiloint2double(__double2hiint(b) ^ (((n + 1) & 2) << 30), __double2loint(b));
-}
 
 // Locates the spline interval of frequency f (ln f = lf) on the log-spaced knots x[0..S-1].
 __device__ __forceinline__ int find_interval(const double* __restrict__ x, int S, double f, double lf, double ln_flo,

@@ -94,6 +94,51 @@ struct DenseWalker {
     DenseMode mode[MBHL_NMODE];
 };
 
+constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + magic - magic = rint(x) for |x| < 2^51
+
+// sin(pi y/2) = y Ps(y^2), cos(pi y/2) = Pc(y^2) on |y| <= 1/2: coefficients from gen_sincos_coeffs.py
+// (Chebyshev-node interpolation in 50-digit arithmetic; max error 2.6e-17 / 1.0e-16 before rounding).
+// Kept in the constant bank so that DFMA reads them as c[][] operands (as immediates each costs two moves per use).
+__constant__ double c_sc[13] = {1.5707963267948966, -0.6459640975062443, 0.07969262624604301, -0.004681754132340976,
+                                0.0001604411507421909, -3.59864335298231e-06, 5.633933781537854e-08,
+                                -1.2337005501361513, 0.25366950789986475, -0.02086348073494657,
+                                0.000919259950041661, -2.520013526428479e-05, 4.6552961874867623e-07};
+#define kS0 c_sc[0]
+#define kS1 c_sc[1]
+#define kS2 c_sc[2]
+#define kS3 c_sc[3]
+#define kS4 c_sc[4]
+#define kS5 c_sc[5]
+#define kS6 c_sc[6]
+#define kC1 c_sc[7]
+#define kC2 c_sc[8]
+#define kC3 c_sc[9]
+#define kC4 c_sc[10]
+#define kC5 c_sc[11]
+#define kC6 c_sc[12]
+
+// sin and cos of p4 quarter turns (angle = p4 pi/2), any |p4| < 2^51.  No conversions, no divides: the
+// nearest integer comes from the magic-number add, the quadrant from the low word of that sum.
+__device__ __forceinline__ void sincos_qturn(double p4, double& sn, double& cs) {
+    const double t = p4 + kRoundMagic;
+    const int n = __double2loint(t);
+    const double y = p4 - (t - kRoundMagic);
+    const double z = y * y;
+    double ps = fma(z, kS6, kS5);
+    double pc = fma(z, kC6, kC5);
+    ps = fma(z, ps, kS4); pc = fma(z, pc, kC4);
+    ps = fma(z, ps, kS3); pc = fma(z, pc, kC3);
+    ps = fma(z, ps, kS2); pc = fma(z, pc, kC2);
+    ps = fma(z, ps, kS1); pc = fma(z, pc, kC1);
+    ps = fma(z, ps, kS0); pc = fma(z, pc, 1.0);
+    ps *= y;
+    const bool odd = (n & 1) != 0;
+    const double a = odd ? pc : ps;      // sin(angle) up to sign
+    const double b = odd ? ps : pc;      // cos(angle) up to sign
+    sn = __hiloint2double(__double2hiint(a) ^ ((n & 2) << 30), __double2loint(a));
+    cs = __hiloint2double(__double2hiint(b) ^ (((n + 1) & 2) << 30), __double2loint(b));
+}
+
 // ---------------------------------------------------------------------------------------------
 // PhenomD pieces (all frequencies are Mf)
 // ---------------------------------------------------------------------------------------------
@@ -241,9 +286,11 @@ __device__ inline double sYlm_theta(int l, int m, double th) {
 // ---------------------------------------------------------------------------------------------
 // Smooth functions of one mode at one frequency: the Q = 8 splined quantities (phase in CYCLES)
 // ---------------------------------------------------------------------------------------------
-__device__ inline double sinc_pi(double u) {   // sin(pi u)/(pi u)
+__device__ inline double sinc_pi(double u) {   // sin(pi u)/(pi u); the quarter-turn sine keeps its relative accuracy near 0
     const double x = kPi * u;
-    return (x == 0.0) ? 1.0 : sinpi(u) / x;
+    double sn, cs;
+    sincos_qturn(2.0 * u, sn, cs);
+    return (x == 0.0) ? 1.0 : sn / x;
 }
 
 __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_hz, double q[MBHL_NQ]) {
@@ -270,7 +317,7 @@ __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_
     const double t = c.t_coal + c.M_s * dpsi * (1.0 / kTwoPi);
     // orbit (O4): positions in light-seconds
     double sa, ca;
-    sincos(kOmega0 * t, &sa, &ca);
+    sincos_qturn(t * (4.0 / kYearSid), sa, ca);                 // alpha = Omega_0 t, in quarter turns
     const double c2a = ca * ca - sa * sa, s2a = 2.0 * sa * ca;
     const double ecc = kArmS / (2.0 * 1.7320508075688772935 * kAuS);
     const double eR = ecc * kAuS;
@@ -303,14 +350,14 @@ __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_
         nPn.re = mc.P[0] * w0 + mc.P[2] * w1 + mc.P[4] * w2 + mc.P[6] * w3 + mc.P[8] * w4 + mc.P[10] * w5;
         nPn.im = mc.P[1] * w0 + mc.P[3] * w1 + mc.P[5] * w2 + mc.P[7] * w3 + mc.P[9] * w4 + mc.P[11] * w5;
         double se, ce;
-        sincospi(-f_hz * (kArmS + kps), &se, &ce);             // exp(-i pi f (L + k.(p_r+p_s)))
+        sincos_qturn(-2.0 * f_hz * (kArmS + kps), se, ce);     // exp(-i pi f (L + k.(p_r+p_s)))
         const cplx e = cmul({ce, se}, nPn);
         gf[a] = cscale(e, sinc_pi(f_hz * kArmS * (1.0 - kn)));
         gb[a] = cscale(e, sinc_pi(f_hz * kArmS * (1.0 + kn)));
     }
     // G_31 = gf[0], G_13 = gb[0], G_21 = gf[1], G_12 = gb[1], G_32 = gf[2], G_23 = gb[2]
     double sz, cz;
-    sincospi(-2.0 * f_hz * kArmS, &sz, &cz);
+    sincos_qturn(-4.0 * f_hz * kArmS, sz, cz);
     const cplx z = {cz, sz};
     const cplx X = csub(cadd(gf[0], cmul(z, gb[0])), cadd(gf[1], cmul(z, gb[1])));
     const cplx Y = csub(cadd(gb[1], cmul(z, gf[1])), cadd(gf[2], cmul(z, gb[2])));

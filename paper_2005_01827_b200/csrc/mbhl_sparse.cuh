@@ -145,8 +145,8 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
     }
     cluster.sync();                                      // both halves of every quantity have landed; no remote access after this
     // B. scaled right-hand sides of the slope system, all rows in parallel
-    for (int idx = tid; idx < kSplineQ * S; idx += kSplineThreads) {
-        const int q = idx / S, r = idx - q * S;
+    for (int q = 0; q < kSplineQ; ++q)
+    for (int r = tid; r < S; r += kSplineThreads) {
         const double* yq = Y + q * SY;
         double v;
         if (r == 0) {
