@@ -308,7 +308,8 @@ def run_dense_sweep(args):
             ms = e0.elapsed_time(e1) / steps
             stage = M.mbhl_stage_times(ctx)
             pairs, bins = M.mbhl_last_work(ctx)
-            flops, flops_table, flops_exec = dense_numerator(pairs, bins, M.mbhl_last_dense_work(ctx))
+            counts = M.mbhl_last_dense_work(ctx)
+            flops, flops_table, flops_exec = dense_numerator(pairs, bins, counts)
             fp64_ms = flops / (fp64_peak * 1e12) * 1e3
             # HBM lower bound: every walker tile (<= 8 walkers) streams at least its largest walker's bins once (80 B per bin),
             # and every record of an in-band interval is read once
@@ -320,7 +321,8 @@ def run_dense_sweep(args):
                                          "stage_ms": {k: float(v) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
                               "roofline": {"bound": "alu" if fp64_ms >= hbm_ms else "hbm", "dense_fp64_bound_ms": fp64_ms, "dense_hbm_bound_ms": hbm_ms,
                                            "frac": max(fp64_ms, hbm_ms) / stage[3], "frac_of_step": max(fp64_ms, hbm_ms) / ms,
-                                           "flops_table": flops_table, "flops_executed": flops_exec, "fp64_peak_tflops": fp64_peak},
+                                           "flops_table": flops_table, "flops_executed": flops_exec, "fp64_peak_tflops": fp64_peak,
+                                           "dense_work_counts": dict(zip(("uniform_calls", "gated_calls", "perbin_record_calls", "lane_evals", "epilogues"), counts))},
                               "finite": bool(torch.isfinite(logL).all().item())}), flush=True)
         M.mbhl_free(ctx)
 
@@ -555,6 +557,7 @@ def run_ours(args):
                      "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": "DFMA-chain probe measured in this run (nominal 148 SM x 64 lanes x 2 x 1.965 GHz = %.1f)" % NOMINAL_FP64_TFLOPS,
                      "algorithmic_flops_per_launch": flops, "flops_table": flops_table, "flops_executed": flops_exec,
+                     "dense_work_counts": dict(zip(("uniform_calls", "gated_calls", "perbin_record_calls", "lane_evals", "epilogues"), counts)),
                      "numerator": "lesser of the SURVEY 8(d) table count and the count executed (k_dense's own tallies, this run)",
                      "dense_ms": dense_ms,
                      "hbm_bound_ms_if_no_reuse": hbm_bytes / (peaks.get("hbm_gbs", 6650.0) * 1e9) * 1e3},
