@@ -1,0 +1,111 @@
+"""Oracle: heterodyned ("relative binning") likelihood, an accuracy-controlled variant of the hot path.
+
+PAPER.md:177 leaves this open ("In the future, we may test different approximations in our GPU implementation to gain
+even more performance"); SURVEY.md 8(f).4 names heterodyned / relative-binning sums.  The definition used here
+(reading H1) follows the algorithm step by step.  TEST INFRASTRUCTURE - see oracle/__init__.py.
+
+Reference parameters Theta0 give, per mode m, a reference phasor on the fine grid
+    E0_m(k) = exp(i theta0_m(f_k))   inside the reference band of mode m, 0 outside,
+theta0_m the total phase of the SPLINE template of Theta0 (Phi - 2 pi f t_coal, O7).  A walker's template is written as
+    h^c(f_k) = sum_m r_{c,m}(f_k) E0_m(k),   r_{c,m}(f) = A_m(f) That^c_m(f) exp(i [theta_m(f) - theta0_m(f)]),
+and r, which is smooth for a walker near Theta0, is replaced on every coarse bin b = [e_b, e_{b+1}) by the straight line
+through its values at the bin's first and last frequency f_L, f_R:  r ~ r0 + r1 (f - fbar), fbar = (f_L + f_R)/2,
+r0 = (r(f_L) + r(f_R))/2, r1 = (r(f_R) - r(f_L))/(f_R - f_L) (0 for a one-bin coarse bin).  Then (eqs. 2, 3, 11)
+    <d|h> ~ Re sum_{c,m,b} [A0 r0 + A1 r1],          A0, A1 = sum_{k in b} w_c conj(d_c) E0_m {1, f_k - fbar},
+    <h|h> ~ Re sum_{c,b} sum_{m,m'} [B0 r0 conj(r0') + B1 (r1 conj(r0') + r0 conj(r1'))],
+                                                      B0, B1 = sum_{k in b} w_c E0_m conj(E0_m') {1, f_k - fbar},
+(the r1 conj(r1') term is second order and dropped).  The summary data A, B are computed once per reference; a walker
+costs its sparse stage plus 2 n_b spline evaluations per mode.  The walker's splines are continued beyond their band
+by the end interval's cubic (the band is taken to be the reference's).  With one fine bin per coarse bin the variant IS
+the brute-force spline likelihood.
+"""
+import math
+
+import numpy as np
+
+from . import likelihood as L
+from . import spline as ospline
+from .constants import MODES
+
+TWO_PI = 2.0 * math.pi
+
+
+def _cycles(Phi, f, t_coal):
+    """Total phase Phi - 2 pi f t_coal in cycles mod 1, the linear term taken exactly (G9), as L._combine does."""
+    lin = np.asarray(f, dtype=np.longdouble) * np.longdouble(t_coal)
+    lin = lin - np.rint(lin)
+    cyc = Phi / TWO_PI
+    return (cyc - np.rint(cyc)) - lin.astype(np.float64)
+
+
+def setup(table, params_ref, freqs, data, psd, S, edges, t0=0.0):
+    """Summary data of the reference Theta0 on the coarse bins given by `edges` (bin indices, 0 ... N)."""
+    freqs = np.asarray(freqs, dtype=np.float64)
+    edges = np.asarray(edges, dtype=np.int64)
+    nb = edges.size - 1
+    w = L.weights(freqs, psd)
+    modes, t_coal = L.sparse_stage(table, params_ref, freqs[0], freqs[-1], S, t0)
+    E0 = np.zeros((len(MODES), freqs.size), dtype=np.complex128)
+    for m, mo in enumerate(modes):
+        if mo is None:
+            continue
+        x = mo["knots"]
+        sel = np.nonzero((freqs >= x[0]) & (freqs <= x[-1]))[0]
+        Phi = ospline.evaluate(x, mo["coef"][:, 1, :], freqs[sel])
+        th = TWO_PI * _cycles(Phi, freqs[sel], t_coal)
+        E0[m, sel] = np.cos(th) + 1j * np.sin(th)
+    fL = freqs[edges[:-1]]
+    fR = freqs[edges[1:] - 1]
+    fbar = 0.5 * (fL + fR)
+    A0 = np.zeros((3, len(MODES), nb), dtype=np.complex128)
+    A1 = np.zeros_like(A0)
+    B0 = np.zeros((3, len(MODES), len(MODES), nb), dtype=np.complex128)
+    B1 = np.zeros_like(B0)
+    for b in range(nb):
+        k = slice(edges[b], edges[b + 1])
+        d = freqs[k] - fbar[b]
+        for c in range(3):
+            wd = w[c, k] * np.conj(data[c, k])
+            for m in range(len(MODES)):
+                A0[c, m, b] = np.sum(wd * E0[m, k])
+                A1[c, m, b] = np.sum(wd * E0[m, k] * d)
+                for mp in range(len(MODES)):
+                    pr = w[c, k] * E0[m, k] * np.conj(E0[mp, k])
+                    B0[c, m, mp, b] = np.sum(pr)
+                    B1[c, m, mp, b] = np.sum(pr * d)
+    return dict(edges=edges, fL=fL, fR=fR, A0=A0, A1=A1, B0=B0, B1=B1, ref_modes=modes, ref_t_coal=t_coal,
+                dd=L.inner(data, data, w), freqs=freqs, S=S, t0=t0)
+
+
+def _envelope(walker_modes, t_coal, summary, f):
+    """r[c, m, :] at frequencies f (extrapolating the splines beyond their bands)."""
+    r = np.zeros((3, len(MODES), f.size), dtype=np.complex128)
+    for m in range(len(MODES)):
+        mo, ref = walker_modes[m], summary["ref_modes"][m]
+        if mo is None or ref is None:
+            continue
+        q = np.stack([ospline.evaluate(mo["knots"], mo["coef"][:, qi, :], f) for qi in range(L.NQ)])
+        Phi0 = ospline.evaluate(ref["knots"], ref["coef"][:, 1, :], f)
+        dth = TWO_PI * (_cycles(q[1], f, t_coal) - _cycles(Phi0, f, summary["ref_t_coal"]))
+        e = q[0] * (np.cos(dth) + 1j * np.sin(dth))
+        for c in range(3):
+            r[c, m] = e * (q[2 + 2 * c] + 1j * q[3 + 2 * c])
+    return r
+
+
+def loglike_parts(table, summary, params):
+    """(<d|h>, <h|h>, logL) of one walker from the summary data (the heterodyned sums above)."""
+    p = L.unpack(params)
+    if not L.walker_valid(p):
+        return 0.0, 0.0, -math.inf
+    modes, t_coal = L.sparse_stage(table, params, summary["freqs"][0], summary["freqs"][-1], summary["S"], summary["t0"])
+    rL = _envelope(modes, t_coal, summary, summary["fL"])
+    rR = _envelope(modes, t_coal, summary, summary["fR"])
+    span = summary["fR"] - summary["fL"]
+    r0 = 0.5 * (rL + rR)
+    r1 = np.where(span > 0.0, (rR - rL) / np.where(span > 0.0, span, 1.0), 0.0)
+    dh = float(np.sum((summary["A0"] * r0 + summary["A1"] * r1).real.astype(np.longdouble)))
+    t = (summary["B0"] * r0[:, :, None, :] * np.conj(r0[:, None, :, :])
+         + summary["B1"] * (r1[:, :, None, :] * np.conj(r0[:, None, :, :]) + r0[:, :, None, :] * np.conj(r1[:, None, :, :])))
+    hh = float(np.sum(t.real.astype(np.longdouble)))
+    return dh, hh, dh - 0.5 * hh - 0.5 * summary["dd"]

@@ -139,3 +139,17 @@ def sparse_batch(batch=16384, seed_offset=3):
     rng = np.random.default_rng(SEED0 + seed_offset)
     T_s = 1.33 * YEAR_JULIAN_S
     return np.stack([draw_prior(rng, None, T_s, M_log_range=(1e5, 1e8)) for _ in range(batch)])
+
+
+def het_edges(freqs, n_coarse):
+    """Coarse-bin edges (bin indices, first 0, last N, strictly increasing) for the heterodyned likelihood variant
+    (row (f).4).  An INPUT of that variant, shared by the oracle and the library: edges are
+    uniform in u(f) = 1/2 [1 - (f^(-5/3) - f_max^(-5/3)) / (f_min^(-5/3) - f_max^(-5/3))] + 1/2 (f - f_min)/(f_max - f_min),
+    i.e. half of the coarse bins follow the leading chirp term of the phase and half the time-shift term."""
+    f = np.asarray(freqs, dtype=np.float64)
+    N = f.size
+    a = f ** (-5.0 / 3.0)
+    u = 0.5 * (1.0 - (a - a[-1]) / (a[0] - a[-1])) + 0.5 * (f - f[0]) / (f[-1] - f[0])
+    e = np.searchsorted(u, np.arange(1, n_coarse) / float(n_coarse), side="left")
+    e = np.unique(np.concatenate([[0], e, [N]]))
+    return e.astype(np.int64)
