@@ -162,6 +162,23 @@ int  mbhl_pt_step(mbhl_pt* pt, int32_t n_steps);                  /* asynchronou
 int  mbhl_pt_state(mbhl_pt* pt, double* theta, double* logL, int64_t* n_accept, int64_t* n_swap);
 void mbhl_pt_free(mbhl_pt* pt);
 
+/* Heterodyned ("relative binning") likelihood - an accuracy-controlled variant of the hot path ("we may
+ * test different approximations in our GPU implementation"; definition: DESIGN.md section 10, reading H1).
+ * mbhl_het_init evaluates the spline template's per-mode phase of the reference parameters params_ref[11] (device
+ * pointer, physical SSB) on the context's grid and accumulates, once, the summary data of the coarse bins
+ * [edges[b], edges[b+1]) (edges: HOST pointer, n_coarse + 1 bin indices, edges[0] = 0 < ... < edges[n_coarse] = N; the
+ * library refines them by the reference's band edges, so that every mode is in band throughout a coarse bin or absent).
+ * mbhl_het_loglike then evaluates walkers from the summary data: per walker the sparse stage (a1-a5) plus
+ * 3 n_coarse spline evaluations per mode, instead of one per fine bin.  The envelope A That exp(i (theta - theta_ref))
+ * is taken piecewise parabolic on the coarse bins (values at a bin's first, centre and last frequency): exact for one
+ * fine bin per coarse bin, third order in the coarse bin width otherwise, accurate for walkers whose phase stays within a fraction of a cycle of the reference's across a
+ * coarse bin (the bulk of a posterior).  The band of a mode is taken to be the reference's; no spline is extrapolated.  d_h, h_h, logL [B]: device
+ * pointers, any may be NULL; asynchronous on the context's stream.  The context must outlive the handle.            */
+typedef struct mbhl_het mbhl_het;
+int  mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const int64_t* edges, int32_t n_coarse);
+int  mbhl_het_loglike(mbhl_het* het, const double* params, int64_t B, double* d_h, double* h_h, double* logL);
+void mbhl_het_free(mbhl_het* het);
+
 /* Noise realisation for fabricating data streams (eq. 12; reading G5 of DESIGN.md): for each channel
  * and bin Re, Im ~ N(0, S_n / (4 df)) independent (the circular Gaussian that eq. 12's "normal modulus, uniform phase"
  * approximates), drawn by Box-Muller from Philox4x32-10 with key = seed and counter (bin, channel, 3, 0).  psd_AET[3][N]

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
 COORDS_PHYSICAL, COORDS_SAMPLED, COORDS_SAMPLED_LISA = 0, 1, 2        # include/mbhl.h MBHL_COORDS_*
-SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free",
+SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free", "mbhl_het_init", "mbhl_het_loglike", "mbhl_het_free",
            "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
            "mbhl_launch_count", "mbhl_last_work", "mbhl_last_dense_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
@@ -55,6 +55,10 @@ def lib():
         L.mbhl_pt_state.argtypes = [vp, vp, vp, vp, vp]
         L.mbhl_pt_free.argtypes = [vp]
         L.mbhl_pt_free.restype = None
+        L.mbhl_het_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32]
+        L.mbhl_het_loglike.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.mbhl_het_free.argtypes = [vp]
+        L.mbhl_het_free.restype = None
         L.mbhl_sparse.argtypes = [vp, vp, i64, vp, vp, vp]
         L.mbhl_workspace_bytes.argtypes = [vp, i64]
         L.mbhl_workspace_bytes.restype = ctypes.c_size_t
@@ -277,3 +281,23 @@ def mbhl_noise(psd_AET, df, seed=0, stream=None):
     out = torch.empty((3, n, 2), dtype=torch.float64, device=psd_AET.device)
     _check(lib().mbhl_noise(_stream_handle(stream), _ptr(psd_AET), n, float(df), ctypes.c_uint64(int(seed)), _ptr(out)))
     return torch.view_as_complex(out)
+
+
+def mbhl_het_init(ctx, params_ref, edges):
+    """Heterodyned-likelihood handle for the reference params_ref [11] (torch CUDA) and coarse-bin edges (int64 numpy, host)."""
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    het = ctypes.c_void_p()
+    _check(lib().mbhl_het_init(ctx, ctypes.byref(het), _ptr(params_ref), ctypes.c_void_p(edges.ctypes.data), int(edges.size - 1)), ctx)
+    return het
+
+
+def mbhl_het_loglike(het, params):
+    """(<d|h>, <h|h>, logL) of the walkers params [B, 11] from the handle's summary data."""
+    B = int(params.shape[0])
+    out = torch.empty((3, B), dtype=torch.float64, device=params.device)
+    _check(lib().mbhl_het_loglike(het, _ptr(params), B, _ptr(out[0]), _ptr(out[1]), _ptr(out[2])))
+    return out[0], out[1], out[2]
+
+
+def mbhl_het_free(het):
+    lib().mbhl_het_free(het)

@@ -5,6 +5,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -603,6 +604,157 @@ void mbhl_pt_free(mbhl_pt* pt) {
     cudaStreamSynchronize(pt->ctx->stream);
     cudaFree(pt->mem);
     delete pt;
+}
+
+// ---------------------------------------------------------------------------------------------
+// heterodyned (relative-binning) likelihood variant
+// ---------------------------------------------------------------------------------------------
+struct mbhl_het {
+    mbhl_ctx* ctx = nullptr;
+    int n_b = 0;
+    char* mem = nullptr;            // one allocation: reference records, edges, summary data
+    double* partials = nullptr;     // [B][n_groups][2], grown on demand
+    size_t partials_bytes = 0;
+    HetEvalArgs E = {};
+};
+
+void mbhl_het_free(mbhl_het* het) {
+    if (!het) return;
+    cudaSetDevice(het->ctx->device);
+    cudaStreamSynchronize(het->ctx->stream);
+    cudaFree(het->mem);
+    cudaFree(het->partials);
+    delete het;
+}
+
+int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const int64_t* edges_host, int32_t n_coarse) {
+    if (!ctx || !out) return MBHL_EINVAL;
+    *out = nullptr;
+    if (!params_ref || !edges_host || n_coarse < 1 || edges_host[0] != 0 || edges_host[n_coarse] != ctx->N)
+        return fail(ctx, MBHL_EINVAL, "mbhl_het_init: need params_ref, edges[0] = 0, edges[n_coarse] = N");
+    for (int b = 0; b < n_coarse; ++b)
+        if (edges_host[b + 1] <= edges_host[b]) return fail(ctx, MBHL_EINVAL, "mbhl_het_init: edges must increase strictly");
+    CU(cudaSetDevice(ctx->device));
+    mbhl_het* het = new (std::nothrow) mbhl_het();
+    if (!het) return MBHL_ENOMEM;
+    het->ctx = ctx;
+    auto bail = [&](int code) { cudaFree(het->mem); delete het; return code; };
+    const int S = ctx->S;
+    cudaStream_t st = ctx->stream;
+    // the reference's sparse stage (a1-a5)
+    char* base;
+    int rc = get_workspace(ctx, 1, &base);
+    if (rc != MBHL_OK) return bail(rc);
+    const WsLayout L = layout(ctx, 1);
+    const bool tm = ctx->timing;
+    ctx->timing = false;
+    rc = run_sparse(ctx, params_ref, 1, MBHL_COORDS_PHYSICAL, base, L, true);
+    ctx->timing = tm;
+    if (rc != MBHL_OK) return bail(rc);
+    WalkerConst wc_host;
+    DenseWalker dw_host;
+    if (cudaMemcpyAsync(&wc_host, base + L.consts, sizeof(WalkerConst), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(&dw_host, base + L.dense, sizeof(DenseWalker), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: copies"));
+    if (!wc_host.valid) return bail(fail(ctx, MBHL_EINVAL, "mbhl_het_init: the reference parameters are outside the model's domain"));
+    // coarse bins actually used: the caller's edges refined by the reference's band edges (reading H1)
+    std::vector<long long> ed(edges_host, edges_host + n_coarse + 1);
+    for (int i = 0; i < MBHL_NMODE; ++i)
+        if (((ctx->mode_mask >> i) & 1u) && dw_host.mode[i].k_hi >= dw_host.mode[i].k_lo) {
+            ed.push_back(dw_host.mode[i].k_lo);
+            ed.push_back((long long)dw_host.mode[i].k_hi + 1);
+        }
+    std::sort(ed.begin(), ed.end());
+    ed.erase(std::unique(ed.begin(), ed.end()), ed.end());
+    n_coarse = (int32_t)ed.size() - 1;
+    het->n_b = n_coarse;
+    const size_t nb = (size_t)n_coarse;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align256(bytes); return o; };
+    const size_t o_wc = take(sizeof(WalkerConst)), o_dw = take(sizeof(DenseWalker)), o_kn = take((size_t)MBHL_NMODE * S * 8);
+    const size_t o_cf = take((size_t)MBHL_NMODE * (S - 1) * kCoefStride * 8), o_ed = take((nb + 1) * 8), o_fl = take(nb * 8), o_fr = take(nb * 8);
+    const size_t o_a0 = take(kHetA * nb * 16), o_a1 = take(kHetA * nb * 16), o_a2 = take(kHetA * nb * 16);
+    const size_t o_b0 = take(kHetB * nb * 16), o_b1 = take(kHetB * nb * 16), o_b2 = take(kHetB * nb * 16);
+    const size_t o_lf = take(MBHL_NMODE * 8), o_id = take(MBHL_NMODE * 8), o_ac = take(MBHL_NMODE * 4), o_lo = take(MBHL_NMODE * 8), o_hi = take(MBHL_NMODE * 8);
+    if (cudaMalloc(&het->mem, off) != cudaSuccess) { cudaGetLastError(); het->mem = nullptr; return bail(fail(ctx, MBHL_ENOMEM, "mbhl_het_init: cudaMalloc")); }
+    char* m = het->mem;
+    if (cudaMemcpyAsync(m + o_wc, base + L.consts, sizeof(WalkerConst), cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_dw, base + L.dense, sizeof(DenseWalker), cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_kn, base + L.knots, (size_t)MBHL_NMODE * S * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_cf, base + L.coef, (size_t)MBHL_NMODE * (S - 1) * kCoefStride * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_ed, ed.data(), (nb + 1) * 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+        return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: copies"));
+    double lf[MBHL_NMODE], id[MBHL_NMODE], flo[MBHL_NMODE], fhi[MBHL_NMODE];
+    int ac[MBHL_NMODE];
+    for (int i = 0; i < MBHL_NMODE; ++i) {
+        lf[i] = wc_host.mode[i].ln_flo; id[i] = wc_host.mode[i].inv_dlog; ac[i] = wc_host.mode[i].active;
+        flo[i] = wc_host.mode[i].f_lo; fhi[i] = wc_host.mode[i].f_hi;
+    }
+    if (cudaMemcpyAsync(m + o_lf, lf, sizeof(lf), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_id, id, sizeof(id), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_ac, ac, sizeof(ac), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_lo, flo, sizeof(flo), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(m + o_hi, fhi, sizeof(fhi), cudaMemcpyHostToDevice, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess)
+        return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: copies"));
+    HetArgs& H = het->E.H;
+    H.tiles = ctx->tiles; H.ref_dw = (const DenseWalker*)(m + o_dw); H.ref_knots = (const double*)(m + o_kn); H.ref_coef = (const double*)(m + o_cf);
+    H.edges = (const long long*)(m + o_ed); H.A0 = (double2*)(m + o_a0); H.A1 = (double2*)(m + o_a1); H.A2 = (double2*)(m + o_a2);
+    H.B0 = (double2*)(m + o_b0); H.B1 = (double2*)(m + o_b1); H.B2 = (double2*)(m + o_b2);
+    H.S = S; H.n_b = n_coarse; H.mode_mask = ctx->mode_mask;
+    het->E.fL = (const double*)(m + o_fl); het->E.fR = (const double*)(m + o_fr);
+    het->E.ref_ln_flo = (const double*)(m + o_lf); het->E.ref_inv_dlog = (const double*)(m + o_id); het->E.ref_active = (const int*)(m + o_ac);
+    het->E.ref_f_lo = (const double*)(m + o_lo); het->E.ref_f_hi = (const double*)(m + o_hi);
+    het->E.n_groups = 3 * ((n_coarse + kHetEvalThreads - 1) / kHetEvalThreads);
+    k_het_edge_freqs<<<(n_coarse + 255) / 256, 256, 0, st>>>(ctx->freqs, H.edges, n_coarse, (double*)(m + o_fl), (double*)(m + o_fr));
+    k_het_summary<<<n_coarse, kHetTile, 0, st>>>(H);
+    ctx->launches += 2;
+    if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: summary kernel"));
+    *out = het;
+    return MBHL_OK;
+}
+
+int mbhl_het_loglike(mbhl_het* het, const double* params, int64_t B, double* d_h, double* h_h, double* logL) {
+    if (!het) return MBHL_EINVAL;
+    mbhl_ctx* ctx = het->ctx;
+    if (B < 0 || (B > 0 && !params)) return fail(ctx, MBHL_EINVAL, "bad params/B");
+    if (B == 0) return MBHL_OK;
+    CU(cudaSetDevice(ctx->device));
+    const bool tm = ctx->timing;
+    for (int64_t o = 0; o < B; o += kSliceBatch) {
+        const int64_t n = (B - o < kSliceBatch) ? (B - o) : kSliceBatch;
+        char* base;
+        int rc = get_workspace(ctx, n, &base);
+        if (rc != MBHL_OK) return rc;
+        const WsLayout L = layout(ctx, n);
+        const size_t need = (size_t)n * het->E.n_groups * 2 * sizeof(double);
+        if (het->partials_bytes < need) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(het->partials);
+            het->partials = nullptr;
+            het->partials_bytes = 0;
+            if (cudaMalloc(&het->partials, need) != cudaSuccess) { cudaGetLastError(); return fail(ctx, MBHL_ENOMEM, "mbhl_het_loglike: cudaMalloc"); }
+            het->partials_bytes = need;
+        }
+        ctx->timing = false;
+        rc = run_sparse(ctx, params + o * MBHL_NPARAM, n, MBHL_COORDS_PHYSICAL, base, L, true);
+        ctx->timing = tm;
+        if (rc != MBHL_OK) return rc;
+        HetEvalArgs E = het->E;
+        E.wc = (const WalkerConst*)(base + L.consts);
+        E.dw = (const DenseWalker*)(base + L.dense);
+        E.knots = (const double*)(base + L.knots);
+        E.coef = (const double*)(base + L.coef);
+        E.partials = het->partials;
+        dim3 g((unsigned)((het->n_b + kHetEvalThreads - 1) / kHetEvalThreads), 3, (unsigned)n);
+        k_het_eval<<<g, kHetEvalThreads, 0, ctx->stream>>>(E);
+        k_final_reduce<<<(unsigned)((n + 3) / 4), 128, 0, ctx->stream>>>(E.dw, E.partials, E.n_groups, n, ctx->dd, d_h ? d_h + o : nullptr,
+                                                                        h_h ? h_h + o : nullptr, logL ? logL + o : nullptr, nullptr, 1);
+        ctx->launches += 2;
+        CU(cudaGetLastError());
+    }
+    return MBHL_OK;
 }
 
 int mbhl_noise(void* stream, const double* psd_AET, int64_t N, double df, uint64_t seed, double* out_AET) {

@@ -270,6 +270,7 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
 }  // namespace mbhl
 
 #include "mbhl_dense.cuh"   // a6 + a7: the fused dense kernel
+#include "mbhl_het.cuh"     // heterodyned likelihood variant
 
 namespace mbhl {
 

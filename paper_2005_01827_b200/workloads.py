@@ -141,15 +141,19 @@ def sparse_batch(batch=16384, seed_offset=3):
     return np.stack([draw_prior(rng, None, T_s, M_log_range=(1e5, 1e8)) for _ in range(batch)])
 
 
-def het_edges(freqs, n_coarse):
+def het_edges(freqs, n_coarse, f_lo=None, f_hi=None):
     """Coarse-bin edges (bin indices, first 0, last N, strictly increasing) for the heterodyned likelihood variant
-    (row (f).4).  An INPUT of that variant, shared by the oracle and the library: edges are
-    uniform in u(f) = 1/2 [1 - (f^(-5/3) - f_max^(-5/3)) / (f_min^(-5/3) - f_max^(-5/3))] + 1/2 (f - f_min)/(f_max - f_min),
-    i.e. half of the coarse bins follow the leading chirp term of the phase and half the time-shift term."""
+    (row (f).4).  An INPUT of that variant, shared by the oracle and the library: half of the
+    n_coarse bins are log-spaced in frequency between f_lo and f_hi (the band the caller expects the signal in, e.g. the
+    first and last knot of the reference's (2,2) mode; default: the whole grid) - the envelope evolves on the scale of
+    f itself at the low end of a band -, the other half uniform in frequency (the time-shift term of the phase)."""
     f = np.asarray(freqs, dtype=np.float64)
     N = f.size
-    a = f ** (-5.0 / 3.0)
-    u = 0.5 * (1.0 - (a - a[-1]) / (a[0] - a[-1])) + 0.5 * (f - f[0]) / (f[-1] - f[0])
-    e = np.searchsorted(u, np.arange(1, n_coarse) / float(n_coarse), side="left")
-    e = np.unique(np.concatenate([[0], e, [N]]))
-    return e.astype(np.int64)
+    f_lo = f[0] if f_lo is None else max(f[0], float(f_lo))
+    f_hi = f[-1] if f_hi is None else min(f[-1], float(f_hi))
+    n1 = max(1, n_coarse // 2)
+    n2 = max(1, n_coarse - n1)
+    e_log = np.searchsorted(f, f_lo * (f_hi / f_lo) ** (np.arange(n1 + 1) / float(n1)), side="left")
+    e_lin = np.searchsorted(f, f[0] + (f[-1] - f[0]) * np.arange(1, n2) / float(n2), side="left")
+    e = np.unique(np.concatenate([[0], e_log, e_lin, [N]]))
+    return e[(e >= 0) & (e <= N)].astype(np.int64)
