@@ -383,6 +383,86 @@ def run_sampler(args):
     M.mbhl_free(ctx)
 
 
+def run_het(args):
+    """the heterodyned likelihood variant against the brute-force path on the BASELINE.json configs[2] data.
+    The batch keeps config 2's shape (1024 walkers in three groups around the three injections) but the walkers are drawn at
+    posterior-like distances from their injection (relative width w; config 2's own 1e-3 is far outside what a heterodyne
+    around ONE reference covers): each group is evaluated against its own reference = its injection.  One JSON line per
+    (width, number of coarse bins): error against the brute-force logL of the same walkers, and throughput."""
+    torch, M, dev, local = _device_setup()
+    from paper_2005_01827_b200 import workloads as W
+    state = {}
+
+    def gpu_template(p, f, S):
+        if "ctx0" not in state:
+            n = f.size
+            state["ctx0"] = M.mbhl_init(torch.as_tensor(f, device=dev), torch.zeros((3, n, 2), dtype=torch.float64, device=dev),
+                                        torch.ones((3, n), dtype=torch.float64, device=dev), sparse_points=S, device=local)
+        h = M.mbhl_template(state["ctx0"], torch.as_tensor(p[None, :].copy(), device=dev))
+        torch.cuda.synchronize()
+        return h[0].cpu().numpy()
+
+    wl = W.build(2, gpu_template)
+    M.mbhl_free(state.pop("ctx0"))
+    t = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=dev)
+    B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
+    ctx = M.mbhl_init(t(wl["freqs"]), t(wl["data"]), t(wl["psd"]), sparse_points=S, t0=wl["t0"], max_batch=B, device=local)
+    inj = wl["injections"]
+    counts = [B - 2 * (B // 3), B // 3, B // 3]
+    kn = M.mbhl_sparse(ctx, t(inj), want_coef=False)[0].cpu().numpy()                # knots of every reference's modes
+    band = [(kn[i][kn[i][:, 0] > 0, 0].min(), kn[i][:, -1].max()) for i in range(3)]    # lowest f_lo, highest f_hi over the modes
+    ev = lambda: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    for width in (1e-7, 1e-6, 1e-5):
+        rng = np.random.default_rng(W.SEED0 + 40)
+        groups = [t(W.perturb(rng, inj[i], counts[i], width)) for i in range(3)]
+        walkers = torch.cat(groups)
+        brute = M.mbhl_loglike_parts(ctx, walkers)
+        e0, e1 = ev()
+        e0.record()
+        for _ in range(args.steps):
+            M.mbhl_loglike_parts(ctx, walkers)
+        e1.record()
+        torch.cuda.synchronize()
+        brute_ms = e0.elapsed_time(e1) / args.steps
+        b_dh, b_hh, b_ll = [x.cpu().numpy() for x in brute]
+        for nb in (512, 2048, 8192):
+            i0, i1 = ev()
+            i0.record()
+            hets = [M.mbhl_het_init(ctx, t(inj[i]), W.het_edges(wl["freqs"], nb, band[i][0], band[i][1])) for i in range(3)]
+            i1.record()
+            torch.cuda.synchronize()
+            outs = [M.mbhl_het_loglike(hets[i], groups[i]) for i in range(3)]
+            for _ in range(3):
+                for i in range(3):
+                    M.mbhl_het_loglike(hets[i], groups[i])
+            launches0 = M.mbhl_launch_count(ctx)
+            e0, e1 = ev()
+            e0.record()
+            for _ in range(args.steps):
+                for i in range(3):
+                    M.mbhl_het_loglike(hets[i], groups[i])
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            launches = M.mbhl_launch_count(ctx) - launches0
+            h_dh, h_hh, h_ll = [np.concatenate([o[j].cpu().numpy() for o in outs]) for j in range(3)]
+            print(json.dumps({
+                "metric": METRIC + " (heterodyned variant)", "value": B / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1, "steps": args.steps,
+                "warmup": 3, "ms_per_step": ms, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"BASELINE.json configs[2] data (N={N}, S={S}); B={B} walkers in three groups at relative width {width:g} around "
+                                       f"their injection, one reference per group, {nb} coarse bins requested",
+                           "walker_width": width, "coarse_bins": nb},
+                "gpu_launches": int(launches),
+                "brute_force": {"ms_per_step": brute_ms, "value": B / (brute_ms * 1e-3)},
+                "speedup_over_brute_force": brute_ms / ms, "summary_ms_per_reference": i0.elapsed_time(i1) / 3.0,
+                "error_vs_brute_force": {"max_abs_dlogL": float(np.max(np.abs(h_ll - b_ll))), "median_abs_dlogL": float(np.median(np.abs(h_ll - b_ll))),
+                                         "max_rel_hh": float(np.max(np.abs(h_hh - b_hh) / b_hh)),
+                                         "max_dh_over_hh": float(np.max(np.abs(h_dh - b_dh) / b_hh))}}), flush=True)
+            for h in hets:
+                M.mbhl_het_free(h)
+    M.mbhl_free(ctx)
+
+
 def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -591,6 +671,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(0, 1, 2, 3, 4),
                     help="BASELINE.json config; 0-2 are likelihood workloads (2 = default bench line), 3 = sparse-stage isolation, "
                          "4 = dense N x B sweep (one JSON line per point)")
+    ap.add_argument("--variant", default="brute", choices=("brute", "het"),
+                    help="het: error-vs-speed table of the heterodyned likelihood variant (SURVEY 8(f).4) on the config-2 data")
     ap.add_argument("--sampler", action="store_true", help="time the parallel-tempered stretch-move ensemble (SURVEY 8(f).2) on the config-2 data")
     ap.add_argument("--batch", type=int, default=0, help="config 3: number of parameter sets (default 16384); config 4: only this batch size")
     ap.add_argument("--logn", type=int, default=0, help="config 4: only the grid with N = 2^logn bins")
@@ -603,6 +685,8 @@ def main():
         if args.config > 2:
             raise SystemExit("--impl reference times the likelihood configs 0-2")
         run_reference(args)
+    elif args.variant == "het":
+        run_het(args)
     elif args.sampler:
         run_sampler(args)
     elif args.config == 3:

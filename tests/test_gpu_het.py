@@ -65,9 +65,10 @@ def test_het_config2_scale_parity_and_accuracy(table):
     inj = wl["injections"][1]
     rng = np.random.default_rng(62)
     walkers = np.concatenate([inj[None, :], W.perturb(rng, inj, 3, 1e-7), W.perturb(rng, inj, 2, 1e-6)])
-    # coarse bins: half of them log-spaced over the band of the reference's (2,2) mode (read from the library's own knots)
-    kn = M.mbhl_sparse(ctx, dev(inj[None, :]), want_coef=False)[0].cpu().numpy()[0, 0]
-    edges = W.het_edges(freqs, 512, kn[0], kn[-1])
+    # coarse bins: half of them log-spaced over the band of the reference's modes (read from the library's own knots)
+    kn = M.mbhl_sparse(ctx, dev(inj[None, :]), want_coef=False)[0].cpu().numpy()[0]
+    f_lo, f_hi = kn[kn[:, 0] > 0, 0].min(), kn[:, -1].max()
+    edges = W.het_edges(freqs, 512, f_lo, f_hi)
     het = M.mbhl_het_init(ctx, dev(inj), edges)
     dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_het_loglike(het, dev(walkers))]
     bdh, bhh, bll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(walkers))]
@@ -81,7 +82,7 @@ def test_het_config2_scale_parity_and_accuracy(table):
         assert abs(hh[b] - rhh) <= tol * rhh and abs(dh[b] - rdh) <= tol * max(abs(rdh), rhh), (b, dh[b], rdh, hh[b], rhh)
     # accuracy against the brute-force path: a small fraction of <h|h>, shrinking with more coarse bins
     err512 = np.max(np.abs(hh - bhh) / bhh)
-    het2 = M.mbhl_het_init(ctx, dev(inj), W.het_edges(freqs, 2048, kn[0], kn[-1]))
+    het2 = M.mbhl_het_init(ctx, dev(inj), W.het_edges(freqs, 2048, f_lo, f_hi))
     dh2, hh2, ll2 = [t.cpu().numpy() for t in M.mbhl_het_loglike(het2, dev(walkers))]
     err2048 = np.max(np.abs(hh2 - bhh) / bhh)
     print('het accuracy at config-2 scale: rel <h|h> error', err512, err2048, 'max |dlogL|', np.max(np.abs(ll - bll)), np.max(np.abs(ll2 - bll)))
