@@ -706,7 +706,7 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
     het->E.fL = (const double*)(m + o_fl); het->E.fR = (const double*)(m + o_fr);
     het->E.ref_ln_flo = (const double*)(m + o_lf); het->E.ref_inv_dlog = (const double*)(m + o_id); het->E.ref_active = (const int*)(m + o_ac);
     het->E.ref_f_lo = (const double*)(m + o_lo); het->E.ref_f_hi = (const double*)(m + o_hi);
-    het->E.n_groups = 3 * ((n_coarse + kHetEvalThreads - 1) / kHetEvalThreads);
+    het->E.n_groups = (n_coarse + kHetEvalThreads - 1) / kHetEvalThreads;
     k_het_edge_freqs<<<(n_coarse + 255) / 256, 256, 0, st>>>(ctx->freqs, H.edges, n_coarse, (double*)(m + o_fl), (double*)(m + o_fr));
     k_het_summary<<<n_coarse, kHetTile, 0, st>>>(H);
     ctx->launches += 2;
@@ -747,7 +747,7 @@ int mbhl_het_loglike(mbhl_het* het, const double* params, int64_t B, double* d_h
         E.knots = (const double*)(base + L.knots);
         E.coef = (const double*)(base + L.coef);
         E.partials = het->partials;
-        dim3 g((unsigned)((het->n_b + kHetEvalThreads - 1) / kHetEvalThreads), 3, (unsigned)n);
+        dim3 g((unsigned)((het->n_b + kHetEvalThreads - 1) / kHetEvalThreads), (unsigned)n);
         k_het_eval<<<g, kHetEvalThreads, 0, ctx->stream>>>(E);
         k_final_reduce<<<(unsigned)((n + 3) / 4), 128, 0, ctx->stream>>>(E.dw, E.partials, E.n_groups, n, ctx->dd, d_h ? d_h + o : nullptr,
                                                                         h_h ? h_h + o : nullptr, logL ? logL + o : nullptr, nullptr, 1);

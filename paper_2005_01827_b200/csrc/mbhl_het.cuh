@@ -11,7 +11,7 @@
 // n = 0, 1, 2, computed ONCE per reference:
 //   k_het_summary   one CTA per coarse bin: a thread per fine bin forms the 6 phasors, then a thread per summary
 //                   entry accumulates it over the tile from shared memory (fixed order: reproducible)
-//   k_het_eval      one thread per (walker, channel, coarse bin): envelope at f_L and f_R (each moved to the nearest
+//   k_het_eval      one thread per (walker, coarse bin): envelope at f_L and f_R (each moved to the nearest
 //                   frequency inside the band common to walker and reference: no spline is extrapolated) for the 6 modes
 //                   from the walker's spline records and the reference's phase records, contraction with A and B, block reduction -> one partial per (walker, block);
 //                   k_final_reduce adds them in fixed order.
@@ -134,77 +134,102 @@ struct HetEvalArgs {
     const double* ref_ln_flo; const double* ref_inv_dlog; const int* ref_active;   // [6]
     const double* ref_f_lo; const double* ref_f_hi;                               // [6] the reference's bands
     double* partials;           // [B][n_groups][2]
-    int n_groups;               // 3 * ceil(n_b / kHetEvalThreads)
+    int n_groups;               // ceil(n_b / kHetEvalThreads)
 };
 
-// envelope r_{c,mi}(f) of one walker: 8 cubics of the walker's record, the reference's phase cubic, one sincos
-__device__ __forceinline__ void het_envelope(const HetEvalArgs& E, int64_t bm, int mi, int c, double f, double lf, double ln_flo,
-                                             double inv_dlog, double& re, double& im) {
-    const int S = E.H.S;
-    const double* x = E.knots + bm * S;
-    const int j = find_interval(x, S, f, lf, ln_flo, inv_dlog);
-    const double u = f - __ldg(x + j);
-    const double* rec = E.coef + (bm * (int64_t)(S - 1) + j) * kCoefStride;
-    auto cubic = [&](int q) {
-        const double2 c01 = __ldg(reinterpret_cast<const double2*>(rec + 4 * q)), c23 = __ldg(reinterpret_cast<const double2*>(rec + 4 * q + 2));
-        return fma(fma(fma(c23.y, u, c23.x), u, c01.y), u, c01.x);
-    };
-    const double p4r = het_ref_phase(E.H.ref_knots + mi * S, E.H.ref_coef + (int64_t)mi * (S - 1) * kCoefStride, S, f, E.ref_ln_flo[mi],
-                                     E.ref_inv_dlog[mi]);
-    double sn, cs;
-    sincos_qturn(cubic(1) - p4r, sn, cs);
-    const double amp = cubic(0), tr = cubic(2 + 2 * c), ti = cubic(3 + 2 * c);
-    const double er = amp * cs, ei = amp * sn;
-    re = er * tr - ei * ti;
-    im = er * ti + ei * tr;
-}
-
-// grid (ceil(n_b / 128), 3, B): thread = coarse bin, blockIdx.y = channel, blockIdx.z = walker
+// grid (ceil(n_b / 128), B): thread = coarse bin, blockIdx.y = walker.  Per mode and evaluation point (first, centre, last
+// frequency of the bin, each moved into the band common to walker and reference) the channel-independent part
+// A exp(i [theta - theta0]) is formed once; the three channels then differ by their transfer cubics only.
 __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
     __shared__ double s_red[2][kHetEvalThreads / 32];
-    const int b = blockIdx.x * kHetEvalThreads + threadIdx.x, c = blockIdx.y;
-    const int64_t wkr = blockIdx.z;
-    const int n_b = E.H.n_b;
+    const int b = blockIdx.x * kHetEvalThreads + threadIdx.x;
+    const int64_t wkr = blockIdx.y;
+    const int n_b = E.H.n_b, S = E.H.S;
     double dh = 0.0, hh = 0.0;
     if (b < n_b && E.wc[wkr].valid) {
         const double fl = E.fL[b], fr = E.fR[b];
         const double fm = 0.5 * (fl + fr), s = 0.5 * (fr - fl);
         const double i1 = s > 0.0 ? 0.5 / s : 0.0, i2 = s > 0.0 ? 0.5 / (s * s) : 0.0;
-        double r0r[MBHL_NMODE], r0i[MBHL_NMODE], r1r[MBHL_NMODE], r1i[MBHL_NMODE], r2r[MBHL_NMODE], r2i[MBHL_NMODE];
+        double er[MBHL_NMODE][3], ei[MBHL_NMODE][3], uu[MBHL_NMODE][3];     // A exp(i dtheta) and u = f - x_j at the three points
+        int jj[MBHL_NMODE][3];                                              // walker interval of each point; -1: mode absent
 #pragma unroll
         for (int mi = 0; mi < MBHL_NMODE; ++mi) {
-            r0r[mi] = r0i[mi] = r1r[mi] = r1i[mi] = r2r[mi] = r2i[mi] = 0.0;
+#pragma unroll
+            for (int p = 0; p < 3; ++p) { er[mi][p] = ei[mi][p] = uu[mi][p] = 0.0; jj[mi][p] = -1; }
             if (!E.ref_active[mi] || !E.wc[wkr].mode[mi].active || !((E.H.mode_mask >> mi) & 1u)) continue;
             const ModeConst& mc = E.wc[wkr].mode[mi];
             const double lo = fmax(mc.f_lo, E.ref_f_lo[mi]), hi = fmin(mc.f_hi, E.ref_f_hi[mi]);
             if (!(lo <= hi)) continue;
-            const double fle = fmin(fmax(fl, lo), hi), fme = fmin(fmax(fm, lo), hi), fre = fmin(fmax(fr, lo), hi);
-            double lr, li, mr, mim, rr, ri;
-            het_envelope(E, wkr * MBHL_NMODE + mi, mi, c, fle, log(fle), mc.ln_flo, mc.inv_dlog, lr, li);
-            het_envelope(E, wkr * MBHL_NMODE + mi, mi, c, fme, log(fme), mc.ln_flo, mc.inv_dlog, mr, mim);
-            het_envelope(E, wkr * MBHL_NMODE + mi, mi, c, fre, log(fre), mc.ln_flo, mc.inv_dlog, rr, ri);
-            r0r[mi] = mr; r0i[mi] = mim;
-            r1r[mi] = (rr - lr) * i1; r1i[mi] = (ri - li) * i1;
-            r2r[mi] = (rr - 2.0 * mr + lr) * i2; r2i[mi] = (ri - 2.0 * mim + li) * i2;
+            const double* x = E.knots + (wkr * MBHL_NMODE + mi) * S;
+            const double* cbase = E.coef + (wkr * MBHL_NMODE + mi) * (int64_t)(S - 1) * kCoefStride;
+#pragma unroll
+            for (int p = 0; p < 3; ++p) {
+                const double f = fmin(fmax(p == 0 ? fl : (p == 1 ? fm : fr), lo), hi);
+                const double lf = log(f);
+                const int j = find_interval(x, S, f, lf, mc.ln_flo, mc.inv_dlog);
+                const double u = f - __ldg(x + j);
+                const double* rec = cbase + (int64_t)j * kCoefStride;
+                const double2 a01 = __ldg(reinterpret_cast<const double2*>(rec)), a23 = __ldg(reinterpret_cast<const double2*>(rec + 2));
+                const double2 p01 = __ldg(reinterpret_cast<const double2*>(rec + 4)), p23 = __ldg(reinterpret_cast<const double2*>(rec + 6));
+                const double amp = fma(fma(fma(a23.y, u, a23.x), u, a01.y), u, a01.x);
+                const double p4w = fma(fma(fma(p23.y, u, p23.x), u, p01.y), u, p01.x);
+                // the reference's phase at the same frequency
+                const double* xr = E.H.ref_knots + mi * S;
+                const int jr = find_interval(xr, S, f, lf, E.ref_ln_flo[mi], E.ref_inv_dlog[mi]);
+                const double ur = f - __ldg(xr + jr);
+                const double* rr = E.H.ref_coef + ((int64_t)mi * (S - 1) + jr) * kCoefStride + 4;
+                const double2 q01 = __ldg(reinterpret_cast<const double2*>(rr)), q23 = __ldg(reinterpret_cast<const double2*>(rr + 2));
+                const double p4r = fma(fma(fma(q23.y, ur, q23.x), ur, q01.y), ur, q01.x);
+                double sn, cs;
+                sincos_qturn(p4w - p4r, sn, cs);
+                er[mi][p] = amp * cs;
+                ei[mi][p] = amp * sn;
+                uu[mi][p] = u;
+                jj[mi][p] = j;
+            }
         }
         // Re(x conj(y)) and Im(x conj(y))
         auto cre = [](double xr, double xi, double yr, double yi) { return xr * yr + xi * yi; };
         auto cim = [](double xr, double xi, double yr, double yi) { return xi * yr - xr * yi; };
+        for (int c = 0; c < 3; ++c) {
+            double r0r[MBHL_NMODE], r0i[MBHL_NMODE], r1r[MBHL_NMODE], r1i[MBHL_NMODE], r2r[MBHL_NMODE], r2i[MBHL_NMODE];
 #pragma unroll
-        for (int mi = 0; mi < MBHL_NMODE; ++mi) {
-            const int64_t ia = (c * MBHL_NMODE + mi) * (int64_t)n_b + b;
-            const double2 a0 = E.H.A0[ia], a1 = E.H.A1[ia], a2 = E.H.A2[ia];
-            dh += (a0.x * r0r[mi] - a0.y * r0i[mi]) + (a1.x * r1r[mi] - a1.y * r1i[mi]) + (a2.x * r2r[mi] - a2.y * r2i[mi]);
+            for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+                double vr[3], vi[3];
 #pragma unroll
-            for (int mp = 0; mp < MBHL_NMODE; ++mp) {
-                const int64_t ib = ((c * MBHL_NMODE + mi) * MBHL_NMODE + mp) * (int64_t)n_b + b;
-                const double2 b0 = E.H.B0[ib], b1 = E.H.B1[ib], b2 = E.H.B2[ib];
-                const double pr = cre(r0r[mi], r0i[mi], r0r[mp], r0i[mp]), pi = cim(r0r[mi], r0i[mi], r0r[mp], r0i[mp]);
-                const double qr = cre(r1r[mi], r1i[mi], r0r[mp], r0i[mp]) + cre(r0r[mi], r0i[mi], r1r[mp], r1i[mp]);
-                const double qi = cim(r1r[mi], r1i[mi], r0r[mp], r0i[mp]) + cim(r0r[mi], r0i[mi], r1r[mp], r1i[mp]);
-                const double sr = cre(r2r[mi], r2i[mi], r0r[mp], r0i[mp]) + cre(r1r[mi], r1i[mi], r1r[mp], r1i[mp]) + cre(r0r[mi], r0i[mi], r2r[mp], r2i[mp]);
-                const double si = cim(r2r[mi], r2i[mi], r0r[mp], r0i[mp]) + cim(r1r[mi], r1i[mi], r1r[mp], r1i[mp]) + cim(r0r[mi], r0i[mi], r2r[mp], r2i[mp]);
-                hh += (b0.x * pr - b0.y * pi) + (b1.x * qr - b1.y * qi) + (b2.x * sr - b2.y * si);
+                for (int p = 0; p < 3; ++p) {
+                    vr[p] = vi[p] = 0.0;
+                    if (jj[mi][p] < 0) continue;
+                    const double* rec = E.coef + ((wkr * MBHL_NMODE + mi) * (int64_t)(S - 1) + jj[mi][p]) * kCoefStride + 8 + 8 * c;
+                    const double u = uu[mi][p];
+                    const double2 t01 = __ldg(reinterpret_cast<const double2*>(rec)), t23 = __ldg(reinterpret_cast<const double2*>(rec + 2));
+                    const double2 s01 = __ldg(reinterpret_cast<const double2*>(rec + 4)), s23 = __ldg(reinterpret_cast<const double2*>(rec + 6));
+                    const double tr = fma(fma(fma(t23.y, u, t23.x), u, t01.y), u, t01.x);
+                    const double ti = fma(fma(fma(s23.y, u, s23.x), u, s01.y), u, s01.x);
+                    vr[p] = er[mi][p] * tr - ei[mi][p] * ti;
+                    vi[p] = er[mi][p] * ti + ei[mi][p] * tr;
+                }
+                r0r[mi] = vr[1]; r0i[mi] = vi[1];
+                r1r[mi] = (vr[2] - vr[0]) * i1; r1i[mi] = (vi[2] - vi[0]) * i1;
+                r2r[mi] = (vr[2] - 2.0 * vr[1] + vr[0]) * i2; r2i[mi] = (vi[2] - 2.0 * vi[1] + vi[0]) * i2;
+            }
+#pragma unroll
+            for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+                const int64_t ia = (c * MBHL_NMODE + mi) * (int64_t)n_b + b;
+                const double2 a0 = E.H.A0[ia], a1 = E.H.A1[ia], a2 = E.H.A2[ia];
+                dh += (a0.x * r0r[mi] - a0.y * r0i[mi]) + (a1.x * r1r[mi] - a1.y * r1i[mi]) + (a2.x * r2r[mi] - a2.y * r2i[mi]);
+                // B_n(m', m) = conj B_n(m, m') and the envelope products are Hermitian too: pairs m' > m count twice
+#pragma unroll
+                for (int mp = mi; mp < MBHL_NMODE; ++mp) {
+                    const int64_t ib = ((c * MBHL_NMODE + mi) * MBHL_NMODE + mp) * (int64_t)n_b + b;
+                    const double2 b0 = E.H.B0[ib], b1 = E.H.B1[ib], b2 = E.H.B2[ib];
+                    const double pr = cre(r0r[mi], r0i[mi], r0r[mp], r0i[mp]), pi = cim(r0r[mi], r0i[mi], r0r[mp], r0i[mp]);
+                    const double qr = cre(r1r[mi], r1i[mi], r0r[mp], r0i[mp]) + cre(r0r[mi], r0i[mi], r1r[mp], r1i[mp]);
+                    const double qi = cim(r1r[mi], r1i[mi], r0r[mp], r0i[mp]) + cim(r0r[mi], r0i[mi], r1r[mp], r1i[mp]);
+                    const double sr = cre(r2r[mi], r2i[mi], r0r[mp], r0i[mp]) + cre(r1r[mi], r1i[mi], r1r[mp], r1i[mp]) + cre(r0r[mi], r0i[mi], r2r[mp], r2i[mp]);
+                    const double si = cim(r2r[mi], r2i[mi], r0r[mp], r0i[mp]) + cim(r1r[mi], r1i[mi], r1r[mp], r1i[mp]) + cim(r0r[mi], r0i[mi], r2r[mp], r2i[mp]);
+                    hh += (mp == mi ? 1.0 : 2.0) * ((b0.x * pr - b0.y * pi) + (b1.x * qr - b1.y * qi) + (b2.x * sr - b2.y * si));
+                }
             }
         }
     }
@@ -219,7 +244,7 @@ __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
         double a = 0.0, h = 0.0;
 #pragma unroll
         for (int i = 0; i < kHetEvalThreads / 32; ++i) { a += s_red[0][i]; h += s_red[1][i]; }
-        double* part = E.partials + (wkr * E.n_groups + (int64_t)c * gridDim.x + blockIdx.x) * 2;
+        double* part = E.partials + (wkr * E.n_groups + blockIdx.x) * 2;
         part[0] = a;
         part[1] = h;
     }
