@@ -10,6 +10,9 @@
  *     interpolation to the dense Fourier grid, mode sum, PSD-weighted inner products,
  *     logL = -1/2 <d-h|d-h> = <d|h> - 1/2 <h|h> - 1/2 <d|d>     (eqs. 2, 3, 11)
  * All arithmetic is fp64 and runs in hand-written sm_100a CUDA kernels; there is no CPU path.
+ * CAVEAT: the model's STRUCTURE is PhenomD/PhenomHM as published, its fit NUMBERS are not: the paper prints none and the
+ * cited tables are not available offline, so model_data/phenomhm_table.csv holds smooth surrogate stand-ins (provenance tag
+ * per entry).  logL will not agree with a real PhenomHM pipeline until that data file is replaced (reading G1).
  * The readings of the paper that fix what is silent or ambiguous are listed in DESIGN.md section 4.
  *
  * Conventions common to all calls
@@ -212,7 +215,7 @@ int mbhl_last_dense_work(mbhl_ctx* ctx, int64_t counts[5]);
 int mbhl_enable_stage_timing(mbhl_ctx* ctx, int32_t on);
 int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]);
 
-/* FP64 DFMA-chain probe used to measure the roofline denominator: each of blocks*threads threads runs
+/* MEASUREMENT AID, not part of the method: FP64 DFMA-chain probe used by bench.py to measure the roofline denominator: each of blocks*threads threads runs
  * iters*8 dependent-chain DFMAs (8 independent chains); sink is a device pointer to >= 1 double.
  * Asynchronous on `stream`.  FLOPs = 2 * blocks * threads * iters * 8.                                   */
 int mbhl_dfma_probe(void* stream, int32_t blocks, int32_t threads, int64_t iters, double* sink);
