@@ -14,7 +14,7 @@
 //      reach row 0 / S-1 use the true not-a-knot rows.
 //        A. 1/h_r; pivots: thread t owns ceil(S/256) rows: c'_r = u_r / (d_r - a_r c'_{r-1}), 1 division per row
 //        B. b_r = rhs_r / (d_r - a_r c'_{r-1}) for 4 quantities, all rows in parallel
-//        C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows)
+//        C. forward sweep g_r = b_r - m_r g_{r-1}   (two warps per quantity, thread = block of ceil(S/64) rows)
 //        D. backward sweep s_r = g_r - c'_r s_{r+1}
 //        E. c_j, d_j of every interval; each thread writes the 32 bytes of one (interval, quantity) with ONE 256-bit
 //           store, a warp 8 full 128-byte lines.
@@ -34,7 +34,7 @@ namespace cg = cooperative_groups;
 __device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
 
 constexpr int kSplineQ = 4;              // quantities per CTA
-constexpr int kSplineThreads = 256;      // 8 warps: evaluation and row-parallel phases; warps 0-3 run the sweeps (one quantity each)
+constexpr int kSplineThreads = 256;      // 8 warps: evaluation, row-parallel phases, and the sweeps (two warps per quantity)
 constexpr int kSplineHaloPivot = 16;
 constexpr int kSplineHaloSweep = 32;
 
@@ -165,12 +165,14 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         A1[q * SP + pad_idx(r)] = v * ivs[pad_idx(r)];
     }
     __syncthreads();
-    // C, D. sweeps in place: warp = quantity, lane = block of rows.  A lane first copies the halo rows it needs
-    // from its neighbour's block into registers, so the neighbour may overwrite them afterwards.
-    if (tid < 32 * kSplineQ) {
-        const int q = tid >> 5, lane = tid & 31;
-        const int m = (S + 31) / 32;
-        const int own0 = lane * m, own1 = min(S, own0 + m);
+    // C, D. sweeps in place.  All 8 warps take part: two warps per quantity, thread = block of ceil(S/64) rows.  A thread
+    // first copies the halo rows it needs from its neighbour's block into registers, so the neighbour may overwrite them
+    // afterwards.  The recurrences are latency chains: the shared-memory operands of 8 steps are loaded first (independent
+    // loads), then the 8 dependent multiply-adds run back to back; rows outside the matrix enter with coefficient 0.
+    {
+        const int q = (tid >> 5) & 3, blk = ((tid >> 7) << 5) | (tid & 31);
+        const int m = (S + 63) / 64;
+        const int own0 = min(S, blk * m), own1 = min(S, own0 + m);
         double* aq = A1 + q * SP;
         double halo[kSplineHaloSweep];
 #pragma unroll
@@ -178,36 +180,68 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
             const int r = own0 - kSplineHaloSweep + i;
             halo[i] = (r >= 0 && r < S) ? aq[pad_idx(r)] : 0.0;
         }
-        __syncwarp();
-        if (own0 < own1) {
+        __syncthreads();
+        {
             double g = 0.0;
 #pragma unroll
-            for (int i = 0; i < kSplineHaloSweep; ++i) {
-                const int r = own0 - kSplineHaloSweep + i;
-                if (r >= 0) g = fma(-mls[pad_idx(r)], g, halo[i]);
+            for (int i0 = 0; i0 < kSplineHaloSweep; i0 += 8) {
+                double mm[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int r = own0 - kSplineHaloSweep + i0 + k;
+                    mm[k] = (r >= 0 && r < S) ? mls[pad_idx(r)] : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) g = fma(-mm[k], g, halo[i0 + k]);
             }
-            for (int r = own0; r < own1; ++r) {
-                g = fma(-mls[pad_idx(r)], g, aq[pad_idx(r)]);
-                aq[pad_idx(r)] = g;
+            for (int r0 = own0; r0 < own1; r0 += 8) {
+                double mm[8], bb[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int r = min(r0 + k, S - 1);
+                    mm[k] = mls[pad_idx(r)];
+                    bb[k] = aq[pad_idx(r)];
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    g = fma(-mm[k], g, bb[k]);
+                    if (r0 + k < own1) aq[pad_idx(r0 + k)] = g;
+                }
             }
         }
-        __syncwarp();
+        __syncthreads();
 #pragma unroll
         for (int i = 0; i < kSplineHaloSweep; ++i) {
             const int r = own1 + i;
             halo[i] = (r < S) ? aq[pad_idx(r)] : 0.0;
         }
-        __syncwarp();
-        if (own0 < own1) {
+        __syncthreads();
+        {
             double sl = 0.0;
 #pragma unroll
-            for (int i = kSplineHaloSweep - 1; i >= 0; --i) {
-                const int r = own1 + i;
-                if (r < S) sl = fma(-cps[pad_idx(r)], sl, halo[i]);
+            for (int i0 = kSplineHaloSweep - 8; i0 >= 0; i0 -= 8) {
+                double cc[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int r = own1 + i0 + k;
+                    cc[k] = (r < S) ? cps[pad_idx(r)] : 0.0;
+                }
+#pragma unroll
+                for (int k = 7; k >= 0; --k) sl = fma(-cc[k], sl, halo[i0 + k]);
             }
-            for (int r = own1 - 1; r >= own0; --r) {
-                sl = fma(-cps[pad_idx(r)], sl, aq[pad_idx(r)]);
-                aq[pad_idx(r)] = sl;
+            for (int r0 = own1 - 1; r0 >= own0; r0 -= 8) {
+                double cc[8], gg[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int r = max(r0 - k, 0);
+                    cc[k] = cps[pad_idx(r)];
+                    gg[k] = aq[pad_idx(r)];
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    sl = fma(-cc[k], sl, gg[k]);
+                    if (r0 - k >= own0) aq[pad_idx(r0 - k)] = sl;
+                }
             }
         }
     }
