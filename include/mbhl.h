@@ -78,7 +78,9 @@ typedef struct mbhl_config {
                                 and right-hand sides); 0 = default 1024 ("~2^10")                    */
     uint32_t mode_mask;      /* bit i enables mode i of the order above; 0 = all six                     */
     double   t0;             /* t_coal = t0 + t_ref                                       */
-    int64_t  max_batch;      /* hint for the internal workspace; 0 = grow on demand                      */
+    int64_t  max_batch;      /* workspace for this many walkers is allocated at init; 0 = grow on demand.  With
+                                max_batch >= B (or a caller workspace) mbhl_loglike* allocates nothing and never
+                                synchronises: the call may be captured in a CUDA graph on the context's stream  */
     int32_t  device;         /* CUDA device ordinal                                                      */
     void*    stream;         /* cudaStream_t all work is enqueued on; NULL = legacy default stream       */
 } mbhl_config;

@@ -364,6 +364,10 @@ int mbhl_init(mbhl_ctx** out, const double* freqs, int64_t N, const double* data
         rc = get_workspace(ctx, cfg->max_batch, &base);
         if (rc != MBHL_OK) return cleanup(rc);
     }
+    // function attributes now, not in the hot path: with max_batch set, mbhl_loglike* then only enqueues kernels and one
+    // memset on the context's stream (no allocation, no synchronisation), so a caller may capture it in a CUDA graph
+    rc = ensure_spline_smem(ctx);
+    if (rc != MBHL_OK) return cleanup(rc);
     cleanup(MBHL_OK);
     *out = ctx;
     return MBHL_OK;

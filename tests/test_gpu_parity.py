@@ -258,6 +258,31 @@ def test_two_live_contexts_with_different_sparse_sizes(table, cfg0):
     M.mbhl_free(c)
 
 
+def test_hot_path_is_capturable_in_a_cuda_graph(table, cfg0):
+    # with max_batch set the call only enqueues kernels and a memset on the context's stream: one graph launch replays it
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        ctx = M.mbhl_init(dev(cfg0["freqs"]), dev(cfg0["data"]), dev(cfg0["psd"]), sparse_points=cfg0["S"], t0=cfg0["t0"],
+                          max_batch=8, stream=s)
+        p = dev(cfg0["params"])
+        out = torch.empty(p.shape[0], dtype=torch.float64, device=DEV)
+        ref = M.mbhl_loglike(ctx, p).clone()
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            M.mbhl_loglike(ctx, p, out)
+        out.zero_()
+        g.replay()
+        s.synchronize()
+        assert torch.equal(out, ref)
+        p[0, 0] *= 1.0001                       # new walker positions in the same buffer: replay evaluates them
+        g.replay()
+        s.synchronize()
+        assert torch.equal(out, M.mbhl_loglike(ctx, p)) and not torch.equal(out, ref)
+        s.synchronize()
+        M.mbhl_free(ctx)
+
+
 def test_init_rejects_bad_grids(cfg0):
     f = cfg0["freqs"][:1000].copy()
     d = np.ascontiguousarray(cfg0["data"][:, :1000])
