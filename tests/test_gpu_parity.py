@@ -167,6 +167,8 @@ def test_noise_free_injection_gives_logl_zero_and_distance_scaling(table):
     inj = wl["injections"][0]
     p = np.stack([inj, inj, inj])
     p[1, 4] *= 2.0
+    # a mass offset large enough to leave the peak: this short grid (T_obs = 0.1 yr, SNR ~ 130) has a posterior width of a
+    # few 1e-5 in ln M_T, so the 1e-5 offset first written here moved logL by less than one unit; 1e-3 is ~30 sigma
     p[2, 0] *= 1.0 + 1e-3
     dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(p))]
     assert abs(ll[0]) < 1e-6 and hh[0] > 1e3
