@@ -413,3 +413,30 @@ def test_narrow_interval_regime_random_masses(table):
             if scale > 0:
                 assert np.max(np.abs(h_gpu[b, c][keep] - h_ref[c][keep])) <= 1e-9 * scale
     M.mbhl_free(ctx)
+
+
+def test_random_grids_knot_counts_and_masses(table):
+    # seeded sweep over what the boundary accepts: grid length, start and spacing, knots per mode, walkers from 1e4 to 3e8
+    # solar masses with mass ratios up to 20 and merger times inside, at the edge of and beyond the observation
+    rng = np.random.default_rng(200501827)
+    worst = 0.0
+    for trial in range(10):
+        N = int(rng.integers(600, 40000))
+        S = int(rng.choice([8, 16, 33, 64, 128, 257, 512]))
+        T_yr = 10.0 ** rng.uniform(-1.5, 0.3)
+        freqs = W.grid(T_yr, N, 10.0 ** rng.uniform(-5.0, -3.3))
+        df = freqs[1] - freqs[0]
+        psd = W.scird_psd_aet(freqs)
+        P = np.stack([W.draw_prior(rng, None, T_yr * W.YEAR_JULIAN_S, q_range=(1.0, 20.0), z_range=(0.5, 10.0), M_log_range=(1e4, 3e8))
+                      for _ in range(5)])
+        P[:, 10] = rng.uniform(0.02, 1.5, 5) * T_yr * W.YEAR_JULIAN_S
+        data = L.template(table, P[0], freqs, S) + W.noise(rng, psd, df)
+        ctx = M.mbhl_init(dev(freqs), dev(data), dev(psd), sparse_points=S)
+        dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(P))]
+        for b in range(P.shape[0]):
+            rdh, rhh, rll = L.loglike_parts(table, P[b], freqs, data, psd, S)
+            assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (trial, N, S, b, ll[b], rll)
+            assert abs(hh[b] - rhh) <= 1e-8 * rhh + 1e-300, (trial, N, S, b, hh[b], rhh)
+            worst = max(worst, abs(ll[b] - rll) / (1.0 + abs(rll)))
+        M.mbhl_free(ctx)
+    assert worst < 1e-9
