@@ -677,7 +677,7 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align256(bytes); return o; };
     const size_t o_wc = take(sizeof(WalkerConst)), o_dw = take(sizeof(DenseWalker)), o_kn = take((size_t)MBHL_NMODE * S * 8);
-    const size_t o_cf = take((size_t)MBHL_NMODE * (S - 1) * kCoefStride * 8), o_ed = take((nb + 1) * 8), o_fl = take(nb * 8), o_fr = take(nb * 8);
+    const size_t o_cf = take((size_t)MBHL_NMODE * (S - 1) * kCoefStride * 8), o_ed = take((nb + 1) * 8), o_pt = take(nb * 6 * 8), o_rp = take((size_t)MBHL_NMODE * nb * 3 * 8), o_pr = take((size_t)MBHL_NMODE * nb * 4);
     const size_t o_a0 = take(kHetA * nb * 16), o_a1 = take(kHetA * nb * 16), o_a2 = take(kHetA * nb * 16);
     const size_t o_b0 = take(kHetB * nb * 16), o_b1 = take(kHetB * nb * 16), o_b2 = take(kHetB * nb * 16);
     const size_t o_lf = take(MBHL_NMODE * 8), o_id = take(MBHL_NMODE * 8), o_ac = take(MBHL_NMODE * 4), o_lo = take(MBHL_NMODE * 8), o_hi = take(MBHL_NMODE * 8);
@@ -707,11 +707,12 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
     H.edges = (const long long*)(m + o_ed); H.A0 = (double2*)(m + o_a0); H.A1 = (double2*)(m + o_a1); H.A2 = (double2*)(m + o_a2);
     H.B0 = (double2*)(m + o_b0); H.B1 = (double2*)(m + o_b1); H.B2 = (double2*)(m + o_b2);
     H.S = S; H.n_b = n_coarse; H.mode_mask = ctx->mode_mask;
-    het->E.fL = (const double*)(m + o_fl); het->E.fR = (const double*)(m + o_fr);
+    het->E.pts = (const double*)(m + o_pt); het->E.ref_p4 = (const double*)(m + o_rp); het->E.present = (const int*)(m + o_pr);
     het->E.ref_ln_flo = (const double*)(m + o_lf); het->E.ref_inv_dlog = (const double*)(m + o_id); het->E.ref_active = (const int*)(m + o_ac);
     het->E.ref_f_lo = (const double*)(m + o_lo); het->E.ref_f_hi = (const double*)(m + o_hi);
     het->E.n_groups = (n_coarse + kHetEvalThreads - 1) / kHetEvalThreads;
-    k_het_edge_freqs<<<(n_coarse + 255) / 256, 256, 0, st>>>(ctx->freqs, H.edges, n_coarse, (double*)(m + o_fl), (double*)(m + o_fr));
+    k_het_bin_points<<<(n_coarse + 127) / 128, 128, 0, st>>>(ctx->freqs, H.edges, n_coarse, H.ref_dw, H.ref_knots, H.ref_coef, S, ctx->mode_mask,
+                                                              (double*)(m + o_pt), (double*)(m + o_rp), (int*)(m + o_pr));
     k_het_summary<<<n_coarse, kHetTile, 0, st>>>(H);
     ctx->launches += 2;
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: summary kernel"));

@@ -48,13 +48,29 @@ __device__ __forceinline__ double het_ref_phase(const double* __restrict__ x, co
     return fma(fma(fma(p23.y, u, p23.x), u, p01.y), u, p01.x);
 }
 
-// fL[b], fR[b]: first and last frequency of coarse bin b
-__global__ void k_het_edge_freqs(const double* __restrict__ freqs, const long long* __restrict__ edges, int n_b, double* __restrict__ fL,
-                                 double* __restrict__ fR) {
+// Per coarse bin b, once per reference: the three evaluation frequencies f_p (first, centre, last), their logarithms, and
+// for every mode present in the bin (the bins are refined by the reference's band edges: present throughout or absent)
+// the reference's phase at the three frequencies in quarter turns.  pts [n_b][3][2] = (f, ln f); ref_p4 [6][n_b][3];
+// present [6][n_b].
+__global__ void k_het_bin_points(const double* __restrict__ freqs, const long long* __restrict__ edges, int n_b, const DenseWalker* __restrict__ ref_dw,
+                                 const double* __restrict__ ref_knots, const double* __restrict__ ref_coef, int S, uint32_t mode_mask,
+                                 double* __restrict__ pts, double* __restrict__ ref_p4, int* __restrict__ present) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= n_b) return;
-    fL[b] = freqs[edges[b]];
-    fR[b] = freqs[edges[b + 1] - 1];
+    const long long k0 = edges[b], k1 = edges[b + 1] - 1;
+    const double fl = freqs[k0], fr = freqs[k1];
+    const double f3[3] = {fl, 0.5 * (fl + fr), fr};
+#pragma unroll
+    for (int p = 0; p < 3; ++p) { pts[(b * 3 + p) * 2] = f3[p]; pts[(b * 3 + p) * 2 + 1] = log(f3[p]); }
+    for (int mi = 0; mi < MBHL_NMODE; ++mi) {
+        const DenseMode dm = ref_dw->mode[mi];
+        const int in = ref_dw->valid && ((mode_mask >> mi) & 1u) && k0 >= dm.k_lo && k1 <= dm.k_hi;
+        present[mi * n_b + b] = in;
+#pragma unroll
+        for (int p = 0; p < 3; ++p)
+            ref_p4[((int64_t)mi * n_b + b) * 3 + p] =
+                in ? het_ref_phase(ref_knots + mi * S, ref_coef + (int64_t)mi * (S - 1) * kCoefStride, S, f3[p], dm.ln_flo, dm.inv_dlog) : 0.0;
+    }
 }
 
 __global__ void __launch_bounds__(kHetTile) k_het_summary(HetArgs H) {
@@ -130,7 +146,9 @@ struct HetEvalArgs {
     const DenseWalker* dw;      // [B]
     const double* knots;        // [B][6][S]
     const double* coef;         // [B][6][S-1][8][4]
-    const double* fL; const double* fR;   // [n_b] first and last frequency of every coarse bin
+    const double* pts;          // [n_b][3][2] (f, ln f) at the first, centre and last frequency of every coarse bin
+    const double* ref_p4;       // [6][n_b][3] the reference's phase there (quarter turns)
+    const int* present;         // [6][n_b] mode in band throughout the coarse bin (else absent: contributes nothing)
     const double* ref_ln_flo; const double* ref_inv_dlog; const int* ref_active;   // [6]
     const double* ref_f_lo; const double* ref_f_hi;                               // [6] the reference's bands
     double* partials;           // [B][n_groups][2]
@@ -147,8 +165,9 @@ __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
     const int n_b = E.H.n_b, S = E.H.S;
     double dh = 0.0, hh = 0.0;
     if (b < n_b && E.wc[wkr].valid) {
-        const double fl = E.fL[b], fr = E.fR[b];
-        const double fm = 0.5 * (fl + fr), s = 0.5 * (fr - fl);
+        const double* pt = E.pts + (int64_t)b * 6;
+        const double f3[3] = {pt[0], pt[2], pt[4]}, lf3[3] = {pt[1], pt[3], pt[5]};
+        const double s = 0.5 * (f3[2] - f3[0]);
         const double i1 = s > 0.0 ? 0.5 / s : 0.0, i2 = s > 0.0 ? 0.5 / (s * s) : 0.0;
         double er[MBHL_NMODE][3], ei[MBHL_NMODE][3], uu[MBHL_NMODE][3];     // A exp(i dtheta) and u = f - x_j at the three points
         int jj[MBHL_NMODE][3];                                              // walker interval of each point; -1: mode absent
@@ -156,16 +175,17 @@ __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
         for (int mi = 0; mi < MBHL_NMODE; ++mi) {
 #pragma unroll
             for (int p = 0; p < 3; ++p) { er[mi][p] = ei[mi][p] = uu[mi][p] = 0.0; jj[mi][p] = -1; }
-            if (!E.ref_active[mi] || !E.wc[wkr].mode[mi].active || !((E.H.mode_mask >> mi) & 1u)) continue;
+            if (!E.present[mi * n_b + b] || !E.wc[wkr].mode[mi].active) continue;
             const ModeConst& mc = E.wc[wkr].mode[mi];
-            const double lo = fmax(mc.f_lo, E.ref_f_lo[mi]), hi = fmin(mc.f_hi, E.ref_f_hi[mi]);
-            if (!(lo <= hi)) continue;
+            if (!(fmax(mc.f_lo, E.ref_f_lo[mi]) <= fmin(mc.f_hi, E.ref_f_hi[mi]))) continue;
             const double* x = E.knots + (wkr * MBHL_NMODE + mi) * S;
             const double* cbase = E.coef + (wkr * MBHL_NMODE + mi) * (int64_t)(S - 1) * kCoefStride;
 #pragma unroll
             for (int p = 0; p < 3; ++p) {
-                const double f = fmin(fmax(p == 0 ? fl : (p == 1 ? fm : fr), lo), hi);
-                const double lf = log(f);
+                // inside the reference's band by construction; moved into the walker's band if it lies outside it
+                const double f = fmin(fmax(f3[p], mc.f_lo), mc.f_hi);
+                const bool moved = f != f3[p];
+                const double lf = moved ? log(f) : lf3[p];
                 const int j = find_interval(x, S, f, lf, mc.ln_flo, mc.inv_dlog);
                 const double u = f - __ldg(x + j);
                 const double* rec = cbase + (int64_t)j * kCoefStride;
@@ -173,13 +193,9 @@ __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
                 const double2 p01 = __ldg(reinterpret_cast<const double2*>(rec + 4)), p23 = __ldg(reinterpret_cast<const double2*>(rec + 6));
                 const double amp = fma(fma(fma(a23.y, u, a23.x), u, a01.y), u, a01.x);
                 const double p4w = fma(fma(fma(p23.y, u, p23.x), u, p01.y), u, p01.x);
-                // the reference's phase at the same frequency
-                const double* xr = E.H.ref_knots + mi * S;
-                const int jr = find_interval(xr, S, f, lf, E.ref_ln_flo[mi], E.ref_inv_dlog[mi]);
-                const double ur = f - __ldg(xr + jr);
-                const double* rr = E.H.ref_coef + ((int64_t)mi * (S - 1) + jr) * kCoefStride + 4;
-                const double2 q01 = __ldg(reinterpret_cast<const double2*>(rr)), q23 = __ldg(reinterpret_cast<const double2*>(rr + 2));
-                const double p4r = fma(fma(fma(q23.y, ur, q23.x), ur, q01.y), ur, q01.x);
+                const double p4r = moved ? het_ref_phase(E.H.ref_knots + mi * S, E.H.ref_coef + (int64_t)mi * (S - 1) * kCoefStride, S, f, E.ref_ln_flo[mi],
+                                                         E.ref_inv_dlog[mi])
+                                         : E.ref_p4[((int64_t)mi * n_b + b) * 3 + p];
                 double sn, cs;
                 sincos_qturn(p4w - p4r, sn, cs);
                 er[mi][p] = amp * cs;
