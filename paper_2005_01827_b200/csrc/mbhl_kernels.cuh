@@ -8,7 +8,10 @@
 namespace mbhl {
 
 constexpr int kCoefStride = MBHL_NQ * 4;   // doubles per (walker, mode, interval) record = 256 B
-constexpr int kDenseThreads = 128;         // 4 warps per CTA
+#ifndef MBHL_DENSE_T
+#define MBHL_DENSE_T 128
+#endif
+constexpr int kDenseThreads = MBHL_DENSE_T;   // 4 warps per CTA
 #ifndef MBHL_DENSE_R
 #define MBHL_DENSE_R 4
 #endif

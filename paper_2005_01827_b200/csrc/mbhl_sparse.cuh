@@ -144,25 +144,32 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         }
     }
     cluster.sync();                                      // both halves of every quantity have landed; no remote access after this
-    // B. scaled right-hand sides of the slope system, all rows in parallel
-    for (int q = 0; q < kSplineQ; ++q)
+    // B. scaled right-hand sides of the slope system, all rows in parallel; a thread takes one row of all 4 quantities
+    // (the spacings and the pivot factor of the row are read once, the 4 right-hand sides are independent chains)
     for (int r = tid; r < S; r += kSplineThreads) {
-        const double* yq = Y + q * SY;
-        double v;
-        if (r == 0) {
-            const double h0 = xk[pad_idx(1)] - xk[pad_idx(0)], h1 = xk[pad_idx(2)] - xk[pad_idx(1)];
-            const double d0 = (yq[1] - yq[0]) * ih[pad_idx(0)], d1 = (yq[2] - yq[1]) * ih[pad_idx(1)];
-            v = ((3.0 * h0 + 2.0 * h1) * h1 * d0 + h0 * h0 * d1) / (h0 + h1);
-        } else if (r == S - 1) {
-            const double hm = xk[pad_idx(S - 1)] - xk[pad_idx(S - 2)], hn = xk[pad_idx(S - 2)] - xk[pad_idx(S - 3)];
-            const double dm = (yq[S - 1] - yq[S - 2]) * ih[pad_idx(S - 2)], dn = (yq[S - 2] - yq[S - 3]) * ih[pad_idx(S - 3)];
-            v = (hm * hm * dn + (2.0 * hn + 3.0 * hm) * hn * dm) / (hn + hm);
+        const double piv = ivs[pad_idx(r)];
+        if (r == 0 || r == S - 1) {
+            const int r0 = (r == 0) ? 0 : S - 3;          // the three knots of the not-a-knot row
+            const double h0 = xk[pad_idx(r0 + 1)] - xk[pad_idx(r0)], h1 = xk[pad_idx(r0 + 2)] - xk[pad_idx(r0 + 1)];
+            const double i0 = ih[pad_idx(r0)], i1 = ih[pad_idx(r0 + 1)];
+#pragma unroll
+            for (int q = 0; q < kSplineQ; ++q) {
+                const double* yq = Y + q * SY;
+                const double d0 = (yq[r0 + 1] - yq[r0]) * i0, d1 = (yq[r0 + 2] - yq[r0 + 1]) * i1;
+                const double v = (r == 0) ? ((3.0 * h0 + 2.0 * h1) * h1 * d0 + h0 * h0 * d1) / (h0 + h1)
+                                          : (h1 * h1 * d0 + (2.0 * h0 + 3.0 * h1) * h0 * d1) / (h0 + h1);
+                A1[q * SP + pad_idx(r)] = v * piv;
+            }
         } else {
             const double hl = xk[pad_idx(r)] - xk[pad_idx(r - 1)], hr = xk[pad_idx(r + 1)] - xk[pad_idx(r)];
-            const double yr = yq[r];
-            v = 3.0 * (hr * ((yr - yq[r - 1]) * ih[pad_idx(r - 1)]) + hl * ((yq[r + 1] - yr) * ih[pad_idx(r)]));
+            const double wl = 3.0 * hr * ih[pad_idx(r - 1)] * piv, wr = 3.0 * hl * ih[pad_idx(r)] * piv;
+#pragma unroll
+            for (int q = 0; q < kSplineQ; ++q) {
+                const double* yq = Y + q * SY;
+                const double yr = yq[r];
+                A1[q * SP + pad_idx(r)] = wl * (yr - yq[r - 1]) + wr * (yq[r + 1] - yr);
+            }
         }
-        A1[q * SP + pad_idx(r)] = v * ivs[pad_idx(r)];
     }
     __syncthreads();
     // C, D. sweeps in place.  All 8 warps take part: two warps per quantity, thread = block of ceil(S/64) rows.  A thread
@@ -246,7 +253,9 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         }
     }
     __syncthreads();
-    // E. coefficients: one (interval, quantity) per thread, one 256-bit store each; 4 consecutive threads write a 128-byte half record
+    // E. coefficients: one (interval, quantity) per thread, one 256-bit store each; 4 consecutive threads write a 128-byte
+    // half record, a warp 8 full lines (a thread per interval writing its whole half record touches 32 lines per store
+    // instruction and was measured slower)
     for (int idx = tid; idx < (S - 1) * kSplineQ; idx += kSplineThreads) {
         const int j = idx >> 2, q = idx & 3;
         const double hinv = ih[pad_idx(j)];
