@@ -352,8 +352,16 @@ __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_
         double se, ce;
         sincos_qturn(-2.0 * f_hz * (kArmS + kps), se, ce);     // exp(-i pi f (L + k.(p_r+p_s)))
         const cplx e = cmul({ce, se}, nPn);
-        gf[a] = cscale(e, sinc_pi(f_hz * kArmS * (1.0 - kn)));
-        gb[a] = cscale(e, sinc_pi(f_hz * kArmS * (1.0 + kn)));
+        // sinc[pi f L (1 -+ k.n)] = sin / x: the two divisions of an arm share one reciprocal
+        const double um = f_hz * kArmS * (1.0 - kn), up = f_hz * kArmS * (1.0 + kn);
+        const double xm = kPi * um, xp = kPi * up;
+        double snm, snp, unused;
+        sincos_qturn(2.0 * um, snm, unused);
+        sincos_qturn(2.0 * up, snp, unused);
+        const double prod = xm * xp;
+        const double inv = 1.0 / prod;
+        gf[a] = cscale(e, (prod != 0.0) ? snm * xp * inv : sinc_pi(um));
+        gb[a] = cscale(e, (prod != 0.0) ? snp * xm * inv : sinc_pi(up));
     }
     // G_31 = gf[0], G_13 = gb[0], G_21 = gf[1], G_12 = gb[1], G_32 = gf[2], G_23 = gb[2]
     double sz, cz;

@@ -134,12 +134,21 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         const int own0 = tid * m, own1 = min(S, own0 + m);
         if (own0 < own1) {
             double cp = 0.0;
-            for (int r = max(0, own0 - kSplineHaloPivot); r < own1; ++r) {
+            int r = max(0, own0 - kSplineHaloPivot);
+            // three consecutive knots roll through registers: one shared-memory load per row
+            double xa = (r > 0) ? xk[pad_idx(r - 1)] : 0.0, xb = xk[pad_idx(r)], xc = (r + 1 < S) ? xk[pad_idx(r + 1)] : 0.0;
+            for (; r < own1; ++r) {
                 double a, d, u;
-                mat(r, a, d, u);
+                if (r == 0 || r == S - 1) {
+                    mat(r, a, d, u);                                 // the not-a-knot rows
+                } else {
+                    const double hl = xb - xa, hr = xc - xb;
+                    a = hr; d = 2.0 * (hl + hr); u = hl;
+                }
                 const double inv = 1.0 / (d - a * cp);
                 cp = u * inv;
                 if (r >= own0) { cps[pad_idx(r)] = cp; ivs[pad_idx(r)] = inv; mls[pad_idx(r)] = a * inv; }
+                xa = xb; xb = xc; xc = (r + 2 < S) ? xk[pad_idx(r + 2)] : 0.0;
             }
         }
     }
