@@ -405,8 +405,9 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                     const int a = max(kt0, m.k_lo), b = min(kt0 + kWarpTile - 1, m.k_hi);
                     const double* x = xk + lane * A.S;
                     const double fa = sf[a - kt0], fb = sf[b - kt0];
-                    ja = find_interval(x, A.S, fa, log(fa), m.ln_flo, m.inv_dlog);
-                    jb = (fb < __ldg(x + ja + 1)) ? ja : find_interval(x, A.S, fb, log(fb), m.ln_flo, m.inv_dlog);
+                    double xh;
+                    ja = find_interval(x, A.S, fa, log(fa), m.ln_flo, m.inv_dlog, &xh);
+                    jb = (fb < xh) ? ja : find_interval(x, A.S, fb, log(fb), m.ln_flo, m.inv_dlog);
                     full = (a == kt0 && b == kt0 + kWarpTile - 1) ? 1 : 0;
                 }
                 while (m_gen) {
@@ -435,9 +436,9 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
 #pragma unroll
                         for (int r = 0; r < kDenseR; ++r) {
                             const int k = kt0 + lane + 32 * r;
-                            int j = ((nrec - 1) * (lane + 32 * r)) / kWarpTile;
-                            while (j > 0 && f[r] < gx[j]) --j;
-                            while (j < nrec - 1 && f[r] >= gx[j + 1]) ++j;
+                            int j = 0;                               // interval of the bin: how many of the staged knots lie at or below it
+#pragma unroll
+                            for (int i = 1; i < kGenSlots; ++i) j += (i < nrec && f[r] >= gx[i]) ? 1 : 0;
                             rec[r] = s_gen + j * kCoefStride;
                             u[r] = f[r] - gx[j];
                             gate[r] = (k >= k_lo && k <= k_hi) ? 1.0 : 0.0;

@@ -236,13 +236,16 @@ struct DenseArgs {
     unsigned long long* work; // [5] executed-work tallies (may be null): see mbhl_last_dense_work
 };
 
-// Locates the spline interval of frequency f (ln f = lf) on the log-spaced knots x[0..S-1].
+// Locates the spline interval of frequency f (ln f = lf) on the log-spaced knots x[0..S-1]; *x_hi receives x[j + 1].
+// The two knots around the guess are loaded together (independent loads: one memory round trip when the guess is right).
 __device__ __forceinline__ int find_interval(const double* __restrict__ x, int S, double f, double lf, double ln_flo,
-                                             double inv_dlog) {
+                                             double inv_dlog, double* x_hi = nullptr) {
     int j = (int)((lf - ln_flo) * inv_dlog);
     j = max(0, min(S - 2, j));
-    while (j > 0 && f < __ldg(x + j)) --j;
-    while (j < S - 2 && f >= __ldg(x + j + 1)) ++j;
+    double xl = __ldg(x + j), xh = __ldg(x + j + 1);
+    while (j > 0 && f < xl) { --j; xh = xl; xl = __ldg(x + j); }
+    while (j < S - 2 && f >= xh) { ++j; xl = xh; xh = __ldg(x + j + 1); }
+    if (x_hi) *x_hi = xh;
     return j;
 }
 
