@@ -446,17 +446,30 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                         mode_perbin(rec, u, gate, h);
                         ++n_rec;
                     } else {
+                        // every bin reads its own record from global memory.  Latency-bound, so the 4 bins of a lane advance in
+                        // phases: the two knots around every bin's guess first (8 independent loads), then the records
                         const int k_lo = w.mode[mi].k_lo, k_hi = w.mode[mi].k_hi;
+                        int jj[kDenseR];
+                        bool in[kDenseR];
+                        double xl[kDenseR], xh[kDenseR];
 #pragma unroll
                         for (int r = 0; r < kDenseR; ++r) {
                             const int k = kt0 + lane + 32 * r;
-                            n_lane += __popc(__ballot_sync(0xffffffffu, k >= k_lo && k <= k_hi));
-                            if (k < k_lo || k > k_hi) continue;
-                            int j = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
-                            while (j > ja_m && f[r] < __ldg(x + j)) --j;
-                            while (j < jb_m && f[r] >= __ldg(x + j + 1)) ++j;
-                            mode_contrib(cbase + (int64_t)j * kCoefStride, f[r] - __ldg(x + j), 1.0, h[r]);
+                            in[r] = k >= k_lo && k <= k_hi;
+                            n_lane += __popc(__ballot_sync(0xffffffffu, in[r]));
+                            jj[r] = ja_m + ((jb_m - ja_m) * (lane + 32 * r)) / kWarpTile;
+                            xl[r] = in[r] ? __ldg(x + jj[r]) : 0.0;
+                            xh[r] = in[r] ? __ldg(x + jj[r] + 1) : 1e300;
                         }
+#pragma unroll
+                        for (int r = 0; r < kDenseR; ++r) {
+                            if (!in[r]) continue;
+                            while (jj[r] > ja_m && f[r] < xl[r]) { --jj[r]; xh[r] = xl[r]; xl[r] = __ldg(x + jj[r]); }
+                            while (jj[r] < jb_m && f[r] >= xh[r]) { ++jj[r]; xl[r] = xh[r]; xh[r] = __ldg(x + jj[r] + 1); }
+                        }
+#pragma unroll
+                        for (int r = 0; r < kDenseR; ++r)
+                            if (in[r]) mode_contrib(cbase + (int64_t)jj[r] * kCoefStride, f[r] - xl[r], 1.0, h[r]);
                     }
                 }
             }
