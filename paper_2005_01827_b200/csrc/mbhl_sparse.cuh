@@ -14,7 +14,8 @@
 //      reach row 0 / S-1 use the true not-a-knot rows.
 //        A. 1/h_r; pivots: thread t owns ceil(S/256) rows: c'_r = u_r / (d_r - a_r c'_{r-1}), 1 division per row
 //        B. b_r = rhs_r / (d_r - a_r c'_{r-1}) for 4 quantities, all rows in parallel
-//        C. forward sweep g_r = b_r - m_r g_{r-1}   (two warps per quantity, thread = block of ceil(S/64) rows)
+//        C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows; operands of 8 steps
+//           are loaded before the 8 dependent multiply-adds)
 //        D. backward sweep s_r = g_r - c'_r s_{r+1}
 //        E. c_j, d_j of every interval; each thread writes the 32 bytes of one (interval, quantity) with ONE 256-bit
 //           store, a warp 8 full 128-byte lines.
@@ -34,9 +35,13 @@ namespace cg = cooperative_groups;
 __device__ __forceinline__ int pad_idx(int r) { return r + (r >> 5); }
 
 constexpr int kSplineQ = 4;              // quantities per CTA
-constexpr int kSplineThreads = 256;      // 8 warps: evaluation, row-parallel phases, and the sweeps (two warps per quantity)
+constexpr int kSplineThreads = 256;      // 8 warps: evaluation and row-parallel phases; 4 of them run the sweeps (one quantity each)
 constexpr int kSplineHaloPivot = 16;
 constexpr int kSplineHaloSweep = 32;
+#ifndef MBHL_SWEEP_BLOCKS
+#define MBHL_SWEEP_BLOCKS 32            // blocks of rows per quantity in the sweeps, one thread each (measured at config 3:
+                                        // 64 blocks 16.9 ms, 32 blocks 16.0 ms, 16 blocks 16.9 ms, 8 blocks 19.2 ms)
+#endif
 
 // Row strides (in doubles) congruent to 4 mod 16: the last phase reads rows q = 0..3 at intervals j..j+3 from one
 // half-warp, and 4 q + j then covers the 16 bank pairs once (a stride of S or S + S/32 + 1 gives 4-way conflicts).
@@ -181,15 +186,18 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         }
     }
     __syncthreads();
-    // C, D. sweeps in place.  All 8 warps take part: two warps per quantity, thread = block of ceil(S/64) rows.  A thread
+    // C, D. sweeps in place: MBHL_SWEEP_BLOCKS threads per quantity, thread = block of rows (the other warps wait).  A thread
     // first copies the halo rows it needs from its neighbour's block into registers, so the neighbour may overwrite them
     // afterwards.  The recurrences are latency chains: the shared-memory operands of 8 steps are loaded first (independent
     // loads), then the 8 dependent multiply-adds run back to back; rows outside the matrix enter with coefficient 0.
     {
-        const int q = (tid >> 5) & 3, blk = ((tid >> 7) << 5) | (tid & 31);
-        const int m = (S + 63) / 64;
-        const int own0 = min(S, blk * m), own1 = min(S, own0 + m);
-        double* aq = A1 + q * SP;
+        // MBHL_SWEEP_BLOCKS blocks of rows per quantity: fewer blocks mean fewer redundant halo rows (instructions), more
+        // blocks a shorter dependent chain
+        constexpr int NB = MBHL_SWEEP_BLOCKS;
+        const int q = tid / NB, blk = tid % NB;
+        const int m = (S + NB - 1) / NB;
+        const int own0 = (tid < kSplineQ * NB) ? min(S, blk * m) : S, own1 = min(S, own0 + m);
+        double* aq = A1 + min(q, kSplineQ - 1) * SP;
         double halo[kSplineHaloSweep];
 #pragma unroll
         for (int i = 0; i < kSplineHaloSweep; ++i) {
