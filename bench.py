@@ -31,10 +31,11 @@ FLOP_PER_BIN = 40.0       # per (walker, active bin) epilo
 # the roofline numerator is the LESSER of the table count and what the kernel EXECUTES.  The executed
 # count is taken per run from the tallies k_dense keeps (mbhl_last_dense_work: evaluator calls, each 4 bins x 32 lanes,
 # in band or not) times the FP64 operations of one evaluation as written in csrc/mbhl_dense.cuh:
-#   one mode at one bin: 48 DFMA + 4 DADD + 4 DMUL = 104 FLOPs (+1 DMUL when the amplitude is gated),
+#   one mode at one bin: 45 DFMA + 4 DADD + 4 DMUL = 98 FLOPs (+1 DMUL when the amplitude is gated); a single-bin evaluation of
+#   the global per-bin path (mode_contrib, the longer sincos polynomials): 48 DFMA + 4 DADD + 5 DMUL = 105 FLOPs,
 #   epilogue per (walker, bin): 12 DFMA + 3 DMUL + 2.75 DADD (per-lane sums and the shuffle tree, per bin) = 29.75 FLOPs.
 # profiles/r02_dense_flop_check.md compares this count with ncu's sm__sass_thread_inst_executed_op_d*_pred_on.
-F_EVAL, F_EVAL_GATED, F_EPI = 104.0, 105.0, 29.75
+F_EVAL, F_EVAL_GATED, F_LANE, F_EPI = 98.0, 99.0, 105.0, 29.75
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_dense launch from the committed `ncu --set full` captures, by config
 DENSE_TRAFFIC = {2: (2.0444e9, "profiles/r02_dense_c2_ncu.txt (dram__bytes_read.sum 2.0350 GB + dram__bytes_write.sum 9.4 MB)")}
@@ -43,7 +44,7 @@ DENSE_TRAFFIC = {2: (2.0444e9, "profiles/r02_dense_c2_ncu.txt (dram__bytes_read.
 def executed_flops(counts):
     """FP64 FLOPs k_dense executed, from its own tallies (uniform, gated, per-bin-record calls; lane evaluations; epilogues)."""
     n_uni, n_gat, n_rec, n_lane, n_epi = counts
-    return 128.0 * (F_EVAL * n_uni + F_EVAL_GATED * (n_gat + n_rec) + F_EPI * n_epi) + F_EVAL_GATED * n_lane
+    return 128.0 * (F_EVAL * n_uni + F_EVAL_GATED * (n_gat + n_rec) + F_EPI * n_epi) + F_LANE * n_lane
 
 
 def dense_numerator(pairs, bins, counts):

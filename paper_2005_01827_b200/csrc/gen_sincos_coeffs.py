@@ -55,3 +55,11 @@ for name, g, fn, odd in (("S", gs, mp.sin, True), ("C", gc, mp.cos, False)):
     print(f"// {name}: max abs error of the rounded polynomial = {mp.nstr(max_err(c, fn, odd), 3)}")
     for k, v in enumerate(c):
         print(f"constexpr double k{name}{k} = {v!r};")
+
+# the shorter pair of the fused dense kernel (sincos_qturn_x in mbhl_dense.cuh, array c_scd): sine of degree 4 and
+# cosine of degree 5 in z; their errors (3.4e-12, 5.6e-14) sit far below the 1e-9 per-bin bar of the template
+for name, g, fn, odd, deg in (("DS", gs, mp.sin, True, 4), ("DC", gc, mp.cos, False, 5)):
+    c = [float(v) for v in cheb_fit(g, deg)]
+    print(f"// {name} (degree {deg}): max abs error of the rounded polynomial = {mp.nstr(max_err(c, fn, odd), 3)}")
+    for k, v in enumerate(c):
+        print(f"constexpr double k{name}{k} = {v!r};")

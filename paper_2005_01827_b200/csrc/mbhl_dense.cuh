@@ -50,7 +50,8 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // sin and cos of p4[r] quarter turns for the kDenseR bins of a lane, advanced in lockstep so that the
-// kDenseR polynomial chains interleave (same arithmetic as sincos_qturn).
+// kDenseR polynomial chains interleave.  Same reduction as sincos_qturn, with the shorter polynomial pair c_scd (sine of
+// degree 4, cosine of degree 5 in y^2: errors 3.4e-12 / 5.6e-14) - every instruction of this loop costs FP64 issue time.
 __device__ __forceinline__ void sincos_qturn_x(const double (&p4)[kDenseR], double (&sn)[kDenseR], double (&cs)[kDenseR]) {
     double y[kDenseR], z[kDenseR], ps[kDenseR], pc[kDenseR];
     int n[kDenseR];
@@ -63,17 +64,15 @@ __device__ __forceinline__ void sincos_qturn_x(const double (&p4)[kDenseR], doub
 #pragma unroll
     for (int r = 0; r < kDenseR; ++r) z[r] = y[r] * y[r];
 #pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], kS6, kS5); pc[r] = fma(z[r], kC6, kC5); }
+    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], c_scd[4], c_scd[3]); pc[r] = fma(z[r], c_scd[10], c_scd[9]); }
 #pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], kS4); pc[r] = fma(z[r], pc[r], kC4); }
+    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], c_scd[2]); pc[r] = fma(z[r], pc[r], c_scd[8]); }
 #pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], kS3); pc[r] = fma(z[r], pc[r], kC3); }
+    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], c_scd[1]); pc[r] = fma(z[r], pc[r], c_scd[7]); }
 #pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], kS2); pc[r] = fma(z[r], pc[r], kC2); }
+    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], c_scd[0]); pc[r] = fma(z[r], pc[r], c_scd[6]); }
 #pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], kS1); pc[r] = fma(z[r], pc[r], kC1); }
-#pragma unroll
-    for (int r = 0; r < kDenseR; ++r) { ps[r] = fma(z[r], ps[r], kS0); pc[r] = fma(z[r], pc[r], 1.0); }
+    for (int r = 0; r < kDenseR; ++r) pc[r] = fma(z[r], pc[r], c_scd[5]);
 #pragma unroll
     for (int r = 0; r < kDenseR; ++r) {
         ps[r] *= y[r];

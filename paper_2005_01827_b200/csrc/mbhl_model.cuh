@@ -103,6 +103,13 @@ __constant__ double c_sc[13] = {1.5707963267948966, -0.6459640975062443, 0.07969
                                 0.0001604411507421909, -3.59864335298231e-06, 5.633933781537854e-08,
                                 -1.2337005501361513, 0.25366950789986475, -0.02086348073494657,
                                 0.000919259950041661, -2.520013526428479e-05, 4.6552961874867623e-07};
+// The shorter pair used per bin by the fused dense kernel (sincos_qturn_x, mbhl_dense.cuh): sine of degree 4 and cosine of
+// degree 5 in y^2 (max error 3.4e-12 / 5.6e-14, gen_sincos_coeffs.py: three multiply-adds fewer per bin, far below the 1e-9
+// per-bin bar of the template).  S0..S4, then C0..C5.
+__constant__ double c_scd[11] = {1.5707963267881, -0.6459640961467954, 0.07969258272563062, -0.004681266256726245,
+                                 0.00015820630355647733,
+                                 0.9999999999999444, -1.2337005501201592, 0.25366950715370434, -0.020863468002244645,
+                                 0.0009191617369539572, -2.4850963357813638e-05};
 #define kS0 c_sc[0]
 #define kS1 c_sc[1]
 #define kS2 c_sc[2]
