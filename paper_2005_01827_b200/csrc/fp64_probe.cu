@@ -4,10 +4,15 @@
 //
 //   build: python -m paper_2005_01827_b200.build --probe      run: paper_2005_01827_b200/fp64_probe
 //
+// Part 1 (operand sources), part 2 (what an instruction of another pipe between two DFMAs costs, and multiply-add chains
+// that share operands) and part 3 (the fast-path body of k_dense, mode_uniform of mbhl_dense.cuh, alone on every SM at the
+// kernel's own occupancy).
 // One CTA on one SM; every warp runs `iters` passes over CH independent dependency chains; the cycle count comes from
 // clock64 around the loop, so the figure is cycles per warp-level instruction per sub-partition (4 per SM).
 #include <cstdio>
 #include <cuda_runtime.h>
+#include "mbhl.h"
+#include "mbhl_kernels.cuh"   // for part 3: the fast-path body of k_dense (mode_uniform) timed in isolation
 
 enum Mode {
     kConst2 = 0,     // x = fma(x, m, e)        m, e loop constants (kept in registers, reused by every instruction)
@@ -111,6 +116,130 @@ static void run(int warps, const double* in) {
     cudaFree(sink); cudaFree(cyc);
 }
 
+// ---- part 2: instruction mix.  12 warps on one SM; every pass issues 8 DFMAs (2 fresh registers + 1 constant: 2.0 cycles
+// each when alone) and, per DFMA, the extra instructions of the mode.  The figure is cycles per DFMA per sub-partition.
+enum Mix { kMixNone = 0, kMixImad = 1, kMixLop3 = 2, kMixFfma = 3, kMix3 = 4, kMac4Shared = 5, kMac4Distinct = 6, kNumMix = 7 };
+
+template <int MODE>
+__global__ void __launch_bounds__(384, 1) k_mix(long iters, const double* __restrict__ in, double* sink, long long* cyc) {
+    double x[8], y[8];
+    unsigned a[8], b[8];
+    float fa[8], fb[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        x[i] = in[threadIdx.x % 32 + 32 * i]; y[i] = in[1024 + threadIdx.x % 32 + 32 * i];
+        a[i] = threadIdx.x * 7 + i; b[i] = threadIdx.x * 13 + i * 5; fa[i] = a[i]; fb[i] = b[i];
+    }
+    const double e = 1e-6;
+    const unsigned pred = threadIdx.x & 1;
+    __syncthreads();
+    const long long t0 = clock64();
+    for (long it = 0; it < iters; ++it) {
+        if (MODE == kMac4Shared) {       // the 4 multiply-adds of a complex product on ONE bin: consecutive instructions share an operand
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                x[0] = fma(y[0], y[2], x[0]); x[1] = fma(y[0], y[3], x[1]); x[0] = fma(-y[1], y[3], x[0]); x[1] = fma(y[1], y[2], x[1]);
+            }
+        } else if (MODE == kMac4Distinct) {   // same dependency structure, no operand shared with the previous instruction
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                x[0] = fma(y[0], y[2], x[0]); x[1] = fma(y[1], y[3], x[1]); x[0] = fma(-y[4], y[5], x[0]); x[1] = fma(y[6], y[7], x[1]);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                x[i] = fma(x[i], y[i], e);
+                if (MODE == kMixImad) a[i] = a[i] * 3 + b[i];
+                if (MODE == kMixLop3) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(b[i]), "r"(pred));
+                if (MODE == kMixFfma) fa[i] = fmaf(fa[i], fb[i], 1.0f);
+                if (MODE == kMix3) { fa[i] = fmaf(fa[i], fb[i], 1.0f); fb[i] = fmaf(fb[i], 0.5f, fa[i]); a[i] = a[i] * 3 + b[i]; }
+            }
+        }
+    }
+    const long long t1 = clock64();
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += x[i] + a[i] + b[i] + fa[i] + fb[i];
+    if (r == 12345.678) sink[0] = r;
+    if ((threadIdx.x & 31) == 0) cyc[threadIdx.x >> 5] = t1 - t0;
+}
+
+static const char* kMixNames[kNumMix] = {
+    "DFMA alone (x = fma(x, y, e))",
+    "DFMA + 1 IMAD (2 register reads)",
+    "DFMA + 1 LOP3 (3 register reads)",
+    "DFMA + 1 FFMA (2 register reads)",
+    "DFMA + 2 FFMA + 1 IMAD",
+    "complex multiply-add, 4-chain on one bin, every instruction shares an operand with the previous one",
+    "complex multiply-add, 4-chain on one bin, no shared operand",
+};
+
+template <int MODE>
+static void run_mix(const double* in) {
+    double* sink; long long* cyc;
+    cudaMalloc(&sink, 64); cudaMalloc(&cyc, 8 * 64);
+    const long iters = 20000;
+    for (int rep = 0; rep < 2; ++rep) { k_mix<MODE><<<1, 384>>>(iters, in, sink, cyc); cudaDeviceSynchronize(); }
+    long long h[12]; cudaMemcpy(h, cyc, 8 * 12, cudaMemcpyDeviceToHost);
+    long long mx = 0; for (int i = 0; i < 12; ++i) if (h[i] > mx) mx = h[i];
+    const int dfma_per_pass = (MODE == kMac4Shared || MODE == kMac4Distinct) ? 32 : 8;
+    printf("  %-100s %.3f cycles per DFMA per sub-partition\n", kMixNames[MODE], (double)mx / ((double)iters * dfma_per_pass * 3));
+    cudaFree(sink); cudaFree(cyc);
+}
+
+// ---- part 3: the fast-path body of k_dense (one mode at the 4 bins of every lane, record in shared memory) alone on the
+// whole GPU at the kernel's occupancy (3 CTAs x 4 warps per SM).  220 FP64 warp instructions per call (u = f - x_j is loop
+// invariant here); 440 cycles per call per sub-partition would be the FP64 pipe's own limit.
+__global__ void __launch_bounds__(128, 3) k_body(int iters, const double* __restrict__ in, double* out, long long* cyc) {
+    extern __shared__ __align__(128) double s_dyn[];
+    double* s_rec = s_dyn;     // 96 records
+    for (int i = threadIdx.x; i < 96 * mbhl::kCoefStride; i += 128) s_rec[i] = in[i % 4096] * 1e-3;
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    double f[mbhl::kDenseR], h[mbhl::kDenseR][6];
+#pragma unroll
+    for (int r = 0; r < mbhl::kDenseR; ++r) {
+        f[r] = 1e-3 + 1e-6 * (lane + 32 * r);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) h[r][i] = 0.0;
+    }
+    const long long t0 = clock64();
+    int slot = threadIdx.x >> 5;
+    for (int it = 0; it < iters; ++it)
+        for (int m = 0; m < 6; ++m) {
+            slot = (slot + 7) % 96;
+            mbhl::mode_uniform<false>(s_rec + slot * mbhl::kCoefStride, 1e-3, f, f, h);
+        }
+    const long long t1 = clock64();
+    double s = 0.0;
+#pragma unroll
+    for (int r = 0; r < mbhl::kDenseR; ++r)
+#pragma unroll
+        for (int i = 0; i < 6; ++i) s += h[r][i];
+    out[blockIdx.x * 128 + threadIdx.x] = s;
+    if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
+}
+
+static void run_body(const double* in, int sms) {
+    const int nb = sms * 3, iters = 20000, smem = 72 * 1024;
+    double* out; long long* cyc;
+    cudaMalloc(&out, 8 * nb * 128); cudaMalloc(&cyc, 8 * nb);
+    cudaFuncSetAttribute(k_body, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    long long mx = 0;
+    for (int rep = 0; rep < 2; ++rep) {
+        k_body<<<nb, 128, smem>>>(iters, in, out, cyc);
+        cudaDeviceSynchronize();
+        long long* hc = new long long[nb];
+        cudaMemcpy(hc, cyc, 8 * nb, cudaMemcpyDeviceToHost);
+        mx = 0;
+        for (int i = 0; i < nb; ++i) if (hc[i] > mx) mx = hc[i];
+        delete[] hc;
+    }
+    printf("  mode_uniform<false> alone, 3 CTAs x 4 warps per SM: %.1f cycles per call per sub-partition (%s)\n",
+           (double)mx / (3.0 * iters * 6), cudaGetErrorString(cudaGetLastError()));
+    cudaFree(out); cudaFree(cyc);
+}
+
 int main() {
     cudaDeviceProp p;
     cudaGetDeviceProperties(&p, 0);
@@ -125,5 +254,10 @@ int main() {
         run<kHorner, 8>(w, in); run<kMacPair, 8>(w, in); run<kAdd2, 8>(w, in); run<kDmma, 8>(w, in); run<kDmmaDfma, 8>(w, in);
         printf("\n");
     }
+    printf("part 2: instruction mix, 12 warps on one SM\n");
+    run_mix<kMixNone>(in); run_mix<kMixImad>(in); run_mix<kMixLop3>(in); run_mix<kMixFfma>(in); run_mix<kMix3>(in);
+    run_mix<kMac4Shared>(in); run_mix<kMac4Distinct>(in);
+    printf("\npart 3: the fast-path body of k_dense in isolation\n");
+    run_body(in, p.multiProcessorCount);
     return 0;
 }

@@ -214,7 +214,7 @@ int run_dense(mbhl_ctx* ctx, int64_t B, char* base, const WsLayout& L, uint32_t 
     if (tm) cudaEventRecord(ctx->ev[3], ctx->stream);
     k_dense<<<(unsigned)((int64_t)P.n_groups * P.n_tiles), kDenseThreads, kDenseSmemBytes, ctx->stream>>>(A);
     if (tm) cudaEventRecord(ctx->ev[4], ctx->stream);
-    k_final_reduce<<<(unsigned)((B + 3) / 4), 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
+    k_final_reduce<<<(unsigned)B, 128, 0, ctx->stream>>>(A.dw, A.partials, A.n_groups, B, ctx->dd, d_h, h_h, logL,
                                                                     count_work ? ctx->counters : nullptr, stride);
     if (tm) { cudaEventRecord(ctx->ev[5], ctx->stream); ctx->n_timed += 1; }
     ctx->launches += 2;
@@ -754,7 +754,7 @@ int mbhl_het_loglike(mbhl_het* het, const double* params, int64_t B, double* d_h
         E.partials = het->partials;
         dim3 g((unsigned)((het->n_b + kHetEvalThreads - 1) / kHetEvalThreads), (unsigned)n);
         k_het_eval<<<g, kHetEvalThreads, 0, ctx->stream>>>(E);
-        k_final_reduce<<<(unsigned)((n + 3) / 4), 128, 0, ctx->stream>>>(E.dw, E.partials, E.n_groups, n, ctx->dd, d_h ? d_h + o : nullptr,
+        k_final_reduce<<<(unsigned)n, 128, 0, ctx->stream>>>(E.dw, E.partials, E.n_groups, n, ctx->dd, d_h ? d_h + o : nullptr,
                                                                         h_h ? h_h + o : nullptr, logL ? logL + o : nullptr, nullptr, 1);
         ctx->launches += 2;
         CU(cudaGetLastError());

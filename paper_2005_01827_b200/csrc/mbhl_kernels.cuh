@@ -280,23 +280,44 @@ __device__ __forceinline__ void mode_contrib(const double* __restrict__ rec, dou
 
 namespace mbhl {
 
-// a7: deterministic final reduction, one warp per walker; logL = <d|h> - 1/2<h|h> - 1/2<d|d> (eq. 2)
+// a7: deterministic final reduction, one CTA (4 warps) per walker; logL = <d|h> - 1/2<h|h> - 1/2<d|d> (eq. 2).
+// Fixed order: thread t takes groups t, t + 128, ...; four independent 16-byte loads are in flight per thread and step
+// (with few walkers and many groups the loop is a chain of L2 round trips), the running sums are added pairwise, then a
+// shuffle tree per warp and the four warp sums in order.
 __global__ void __launch_bounds__(128) k_final_reduce(const DenseWalker* __restrict__ dw, const double* __restrict__ partials,
                                                       int n_groups, int64_t B, double dd, double* __restrict__ d_h,
                                                       double* __restrict__ h_h, double* __restrict__ logL,
                                                       unsigned long long* __restrict__ counters, int64_t stride) {
-    const int64_t b = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (b >= B) return;
-    const int lane = threadIdx.x & 31;
-    const double* p = partials + b * n_groups * 2;
-    double sdh = 0.0, shh = 0.0;
-    for (int i = lane; i < n_groups; i += 32) { sdh += p[2 * i]; shh += p[2 * i + 1]; }
+    __shared__ double s_w[4][2];
+    const int64_t b = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double2* p2 = reinterpret_cast<const double2*>(partials + b * n_groups * 2);
+    double2 acc[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc[k] = make_double2(0.0, 0.0);
+    int i = tid;
+    for (; i + 384 < n_groups; i += 512) {
+        double2 v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = p2[i + 128 * k];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { acc[k].x += v[k].x; acc[k].y += v[k].y; }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        if (i + 128 * k < n_groups) { const double2 v = p2[i + 128 * k]; acc[k].x += v.x; acc[k].y += v.y; }
+    double sdh = (acc[0].x + acc[1].x) + (acc[2].x + acc[3].x);
+    double shh = (acc[0].y + acc[1].y) + (acc[2].y + acc[3].y);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         sdh += __shfl_down_sync(0xffffffffu, sdh, o);
         shh += __shfl_down_sync(0xffffffffu, shh, o);
     }
-    if (lane == 0) {
+    if (lane == 0) { s_w[warp][0] = sdh; s_w[warp][1] = shh; }
+    __syncthreads();
+    if (tid == 0) {
+        sdh = (s_w[0][0] + s_w[1][0]) + (s_w[2][0] + s_w[3][0]);
+        shh = (s_w[0][1] + s_w[1][1]) + (s_w[2][1] + s_w[3][1]);
         const bool valid = dw[b].valid != 0;
         if (!valid) { sdh = 0.0; shh = 0.0; }
         if (d_h) d_h[b * stride] = sdh;

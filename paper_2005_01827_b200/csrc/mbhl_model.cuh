@@ -209,7 +209,7 @@ __device__ inline void psi_ins_raw(const WalkerConst& c, double f, double* psi, 
     // d/df [c_i v^(i-5)] = v^(i-5)/f * ((i-5)/3 c_i + f c_i'), with f c_5' = ph5, f c_6' = -6848/63
     const double dS = (-5.0 / 3.0) + (-1.0) * c.ph[2] * v2 + (-2.0 / 3.0) * c.ph[3] * v3 + (-1.0 / 3.0) * c.ph[4] * v4 +
                       c.ph[5] * v5 + ((1.0 / 3.0) * c6 - 6848.0 / 63.0) * v6 + (2.0 / 3.0) * c.ph[7] * v7;
-    const double f13 = cbrt(f), f23 = f13 * f13;
+    const double f13 = v * 0.68278406325529568147, f23 = f13 * f13;     // cbrt(f) = cbrt(pi f) / cbrt(pi): one cube root fewer
     *psi = -0.25 * kPi + c.pre * iv5 * S +
            (c.sig[0] * f + 0.75 * c.sig[1] * f * f13 + 0.6 * c.sig[2] * f * f23 + 0.5 * c.sig[3] * f * f) * c.inveta;
     *dpsi = c.pre * iv5 * dS * invf + (c.sig[0] + c.sig[1] * f13 + c.sig[2] * f23 + c.sig[3] * f) * c.inveta;
@@ -267,9 +267,8 @@ __device__ inline double t_of_f(const WalkerConst& c, int mi, double f_hz) {
 // ---------------------------------------------------------------------------------------------
 // Spin-weight -2 spherical harmonics needed by the six modes (closed forms), theta = iota
 // ---------------------------------------------------------------------------------------------
-__device__ inline double sYlm_theta(int l, int m, double th) {
-    const double ct = cos(th), st = sin(th);
-    const double ch = cos(0.5 * th), sh = sin(0.5 * th);
+// ct, st = cos, sin of theta; ch, sh = cos, sin of theta / 2 (the caller evaluates them once for both signs of m)
+__device__ inline double sYlm_theta(int l, int m, double ct, double st, double ch, double sh) {
     const double ch2 = ch * ch, sh2 = sh * sh;
     if (l == 2) {
         if (m == 2) return sqrt(5.0 / (64.0 * kPi)) * (1.0 + ct) * (1.0 + ct);
@@ -493,12 +492,13 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     double frd[MBHL_NMODE], fdm[MBHL_NMODE];
     {
         const double oma = 1.0 - af;
+        const double ln_oma = log(oma);                       // (1 - a_f)^p = exp(p ln(1 - a_f)): one logarithm serves the 4 powers
         const double inv = 1.0 / (kTwoPi * (1.0 - Erad));
         for (int mi = 0; mi < mode_hi; ++mi) {
             if (mi != 0 && mi < mode_lo) continue;           // mode (2,2) is needed by everyone
             const double* t6 = T + MT_qnm_22_f1 + 6 * mi;
-            const double om = t6[0] + t6[1] * pow(oma, t6[2]);
-            const double Q = t6[3] + t6[4] * pow(oma, t6[5]);
+            const double om = t6[0] + t6[1] * exp(t6[2] * ln_oma);
+            const double Q = t6[3] + t6[4] * exp(t6[5] * ln_oma);
             frd[mi] = om * inv;
             fdm[mi] = frd[mi] / (2.0 * Q);
         }
@@ -528,38 +528,39 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     c.alp[3] = fit11(MT_pd_alpha4_l00, eta, x);
     c.alp[4] = fit11(MT_pd_alpha5_l00, eta, x);
 
-    // PN phase coefficients
+    // PN phase coefficients (constant ratios are written (K / D) * x so that they fold at compile time: K * x / D is a
+    // run-time division, and this routine is one long dependent chain)
     c.ph[0] = 1.0;
     c.ph[1] = 0.0;
-    c.ph[2] = 3715.0 / 756.0 + 55.0 * eta / 9.0;
-    c.ph[3] = -16.0 * kPi + 113.0 * delta * xa / 3.0 + (113.0 / 3.0 - 76.0 * eta / 3.0) * xs;
-    c.ph[4] = 15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * e2 / 72.0 + (-405.0 / 8.0 + 200.0 * eta) * xa * xa -
-              (405.0 / 4.0) * delta * xa * xs + (-405.0 / 8.0 + 5.0 * eta / 2.0) * xs * xs;
-    c.ph[5] = 38645.0 * kPi / 756.0 - 65.0 * kPi * eta / 9.0 + delta * (-732985.0 / 2268.0 - 140.0 * eta / 9.0) * xa +
-              (-732985.0 / 2268.0 + 24260.0 * eta / 81.0 + 340.0 * e2 / 9.0) * xs;
+    c.ph[2] = 3715.0 / 756.0 + (55.0 / 9.0) * eta;
+    c.ph[3] = -16.0 * kPi + (113.0 / 3.0) * delta * xa + (113.0 / 3.0 - (76.0 / 3.0) * eta) * xs;
+    c.ph[4] = 15293365.0 / 508032.0 + (27145.0 / 504.0) * eta + (3085.0 / 72.0) * e2 + (-405.0 / 8.0 + 200.0 * eta) * xa * xa -
+              (405.0 / 4.0) * delta * xa * xs + (-405.0 / 8.0 + (5.0 / 2.0) * eta) * xs * xs;
+    c.ph[5] = 38645.0 * kPi / 756.0 - (65.0 * kPi / 9.0) * eta + delta * (-732985.0 / 2268.0 - (140.0 / 9.0) * eta) * xa +
+              (-732985.0 / 2268.0 + (24260.0 / 81.0) * eta + (340.0 / 9.0) * e2) * xs;
     c.ph[6] = 11583231236531.0 / 4694215680.0 - 6848.0 * kEulerGamma / 21.0 - 640.0 * kPi * kPi / 3.0 +
-              (-15737765635.0 / 3048192.0 + 2255.0 * kPi * kPi / 12.0) * eta + 76055.0 * e2 / 1728.0 - 127825.0 * e3 / 1296.0 +
+              (-15737765635.0 / 3048192.0 + 2255.0 * kPi * kPi / 12.0) * eta + (76055.0 / 1728.0) * e2 - (127825.0 / 1296.0) * e3 +
               (2270.0 * kPi / 3.0) * delta * xa + (2270.0 * kPi / 3.0 - 520.0 * kPi * eta) * xs;
-    c.ph[7] = 77096675.0 * kPi / 254016.0 + 378515.0 * kPi * eta / 1512.0 - 74045.0 * kPi * e2 / 756.0 +
-              delta * (-25150083775.0 / 3048192.0 + 26804935.0 * eta / 6048.0 - 1985.0 * e2 / 48.0) * xa +
-              (-25150083775.0 / 3048192.0 + 10566655595.0 * eta / 762048.0 - 1042165.0 * e2 / 3024.0 + 5345.0 * e3 / 36.0) * xs;
+    c.ph[7] = 77096675.0 * kPi / 254016.0 + (378515.0 * kPi / 1512.0) * eta - (74045.0 * kPi / 756.0) * e2 +
+              delta * (-25150083775.0 / 3048192.0 + (26804935.0 / 6048.0) * eta - (1985.0 / 48.0) * e2) * xa +
+              (-25150083775.0 / 3048192.0 + (10566655595.0 / 762048.0) * eta - (1042165.0 / 3024.0) * e2 + (5345.0 / 36.0) * e3) * xs;
     // PN amplitude coefficients, premultiplied by pi^(i/3)
     {
         double a[7];
         a[0] = 1.0;
         a[1] = 0.0;
-        a[2] = -323.0 / 224.0 + 451.0 * eta / 168.0;
-        a[3] = 27.0 * delta * xa / 8.0 + (27.0 / 8.0 - 11.0 * eta / 6.0) * xs;
-        a[4] = -27312085.0 / 8128512.0 - 1975055.0 * eta / 338688.0 + 105271.0 * e2 / 24192.0 + (-81.0 / 32.0 + 8.0 * eta) * xa * xa -
-               (81.0 / 16.0) * delta * xa * xs + (-81.0 / 32.0 + 17.0 * eta / 8.0) * xs * xs;
-        a[5] = -85.0 * kPi / 64.0 + 85.0 * kPi * eta / 16.0 + delta * (285197.0 / 16128.0 - 1579.0 * eta / 4032.0) * xa +
-               (285197.0 / 16128.0 - 15317.0 * eta / 672.0 - 2227.0 * e2 / 1008.0) * xs;
+        a[2] = -323.0 / 224.0 + (451.0 / 168.0) * eta;
+        a[3] = (27.0 / 8.0) * delta * xa + (27.0 / 8.0 - (11.0 / 6.0) * eta) * xs;
+        a[4] = -27312085.0 / 8128512.0 - (1975055.0 / 338688.0) * eta + (105271.0 / 24192.0) * e2 + (-81.0 / 32.0 + 8.0 * eta) * xa * xa -
+               (81.0 / 16.0) * delta * xa * xs + (-81.0 / 32.0 + (17.0 / 8.0) * eta) * xs * xs;
+        a[5] = -85.0 * kPi / 64.0 + (85.0 * kPi / 16.0) * eta + delta * (285197.0 / 16128.0 - (1579.0 / 4032.0) * eta) * xa +
+               (285197.0 / 16128.0 - (15317.0 / 672.0) * eta - (2227.0 / 1008.0) * e2) * xs;
         a[6] = -177520268561.0 / 8583708672.0 + (545384828789.0 / 5007163392.0 - 205.0 * kPi * kPi / 48.0) * eta -
-               3248849057.0 * e2 / 178827264.0 + 34473079.0 * e3 / 6386688.0 +
-               (1614569.0 / 64512.0 - 1873643.0 * eta / 16128.0 + 2167.0 * e2 / 42.0) * xa * xa +
-               (31.0 * kPi / 12.0 - 7.0 * kPi * eta / 3.0) * xs +
-               (1614569.0 / 64512.0 - 61391.0 * eta / 1344.0 + 57451.0 * e2 / 4032.0) * xs * xs +
-               delta * xa * (31.0 * kPi / 12.0 + (1614569.0 / 32256.0 - 165961.0 * eta / 2688.0) * xs);
+               (3248849057.0 / 178827264.0) * e2 + (34473079.0 / 6386688.0) * e3 +
+               (1614569.0 / 64512.0 - (1873643.0 / 16128.0) * eta + (2167.0 / 42.0) * e2) * xa * xa +
+               (31.0 * kPi / 12.0 - (7.0 * kPi / 3.0) * eta) * xs +
+               (1614569.0 / 64512.0 - (61391.0 / 1344.0) * eta + (57451.0 / 4032.0) * e2) * xs * xs +
+               delta * xa * (31.0 * kPi / 12.0 + (1614569.0 / 32256.0 - (165961.0 / 2688.0) * eta) * xs);
         const double pi13 = cbrt(kPi);
         double pw = 1.0;
         for (int i = 0; i < 7; ++i) { c.am[i] = a[i] * pw; pw *= pi13; }
@@ -587,10 +588,12 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
     }
     {
         // f_ref: root of g(f) = (5/6)/f - 2x/(x^2+w^2) - gamma2/w above f_peak (reading G4)
-        const double w = c.w, g2w = c.gam2ow;
+        // multiplied through by f (x^2 + w^2) > 0: same sign and root, no division in the iteration
+        const double w = c.w, g2w = c.gam2ow, fRD = c.fRD;
         auto g = [&](double f) {
-            const double xx = f - c.fRD;
-            return (5.0 / 6.0) / f - 2.0 * xx / (xx * xx + w * w) - g2w;
+            const double xx = f - fRD;
+            const double den = fma(xx, xx, w * w);
+            return fma(5.0 / 6.0, den, -f * fma(g2w, den, 2.0 * xx));
         };
         double lo = c.f_peak, hi = c.fRD + 4.0 * w;
         for (int it = 0; it < 64 && g(hi) > 0.0; ++it) hi += w;
@@ -678,7 +681,10 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
         mc.ampc = ampbase * fabs(clm * massf);
         mc.vpow = vp;
         // mode polarisation tensor P_lm = 1/2 Y_{l,-m}(P+ + i Px) + 1/2 (-1)^l conj(Y_lm)(P+ - i Px)
-        const double ym = sYlm_theta(l, -m, inc), yp = sYlm_theta(l, m, inc);
+        double ct_i, st_i, ch_i, sh_i;
+        sincos(inc, &st_i, &ct_i);
+        sincos(0.5 * inc, &sh_i, &ch_i);
+        const double ym = sYlm_theta(l, -m, ct_i, st_i, ch_i, sh_i), yp = sYlm_theta(l, m, ct_i, st_i, ch_i, sh_i);
         double sm, cm;
         sincos(m * phi_ref, &sm, &cm);
         const cplx Ym = {ym * cm, -ym * sm};                 // Y_{l,-m} = y e^{-i m phi}
@@ -718,13 +724,14 @@ __device__ inline void build_walker(const double* __restrict__ p, double t0, dou
                 // the time to coalescence tau = t_coal - t_22 falls off like x^(-8/3) (P6), so tau^(-3/8) is nearly
                 // linear in x: the secant steps run on g(x) = tau(x)^(-3/8) - t_coal^(-3/8), which has the sign of t_22
                 const double xa = mc.aP[0] * (f_min * c.M_s);        // t22(xa) = t_min < 0 <= t_top
-                const double g0 = pow(c.t_coal, -0.375);
+                auto p38 = [](double tau) { return exp(-0.375 * log(tau)); };     // tau^(-3/8); only the sign and zero of g matter
+                const double g0 = p38(c.t_coal);
                 auto g = [&](double x22) {
                     const double tau = c.t_coal - t22(x22);
-                    return (tau > 0.0) ? pow(tau, -0.375) - g0 : 1e300;
+                    return (tau > 0.0) ? p38(tau) - g0 : 1e300;
                 };
-                const double ga = pow(c.t_coal - t_min, -0.375) - g0;
-                const double gb = (c.t_coal - t_top > 0.0) ? pow(c.t_coal - t_top, -0.375) - g0 : 1e300;
+                const double ga = p38(c.t_coal - t_min) - g0;
+                const double gb = (c.t_coal - t_top > 0.0) ? p38(c.t_coal - t_top) - g0 : 1e300;
                 x0 = bracketed_root(g, xa, ga, kFPhiIns, gb, 4e-16 * g0);
             }
             f_lo = fmax(f_min, x0 * (0.5 * m) / c.M_s);
