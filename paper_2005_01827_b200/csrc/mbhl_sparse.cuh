@@ -186,11 +186,74 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         }
     }
     __syncthreads();
-    // C, D. sweeps in place: MBHL_SWEEP_BLOCKS threads per quantity, thread = block of rows (the other warps wait).  A thread
-    // first copies the halo rows it needs from its neighbour's block into registers, so the neighbour may overwrite them
-    // afterwards.  The recurrences are latency chains: the shared-memory operands of 8 steps are loaded first (independent
-    // loads), then the 8 dependent multiply-adds run back to back; rows outside the matrix enter with coefficient 0.
-    {
+    // C, D. sweeps in place.  A thread owns a block of consecutive rows and first copies the halo rows it needs from its
+    // neighbour's block into registers, so the neighbour may overwrite them afterwards.  The recurrences are latency chains:
+    // the shared-memory operands of 8 steps are loaded first (independent loads), then the 8 dependent multiply-adds run back
+    // to back.
+    if ((S & 31) == 0 && S <= 1024) {
+        // The usual case (S = 256, 512, 1024): blocks of exactly 32 rows, warp = quantity, lane = block.  Row 32 blk + k sits
+        // at padded index 33 blk + k, so a block and its neighbours are addressed with compile-time offsets from one base
+        // and nothing is bounds-checked: this phase was a fifth of the kernel's instructions, none of them FP64.
+        const int nblk = S >> 5;
+        const int q = tid >> 5, blk = tid & 31;
+        const bool on = q < kSplineQ && blk < nblk;
+        double* const aq = A1 + min(q, kSplineQ - 1) * SP + min(blk, nblk - 1) * 33;
+        const double* const mq = mls + min(blk, nblk - 1) * 33;
+        const double* const cq = cps + min(blk, nblk - 1) * 33;
+        const bool has_prev = on && blk > 0, has_next = on && blk + 1 < nblk;
+        double halo[32];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) halo[k] = has_prev ? aq[k - 33] : 0.0;
+        __syncthreads();
+        if (on) {
+            double g = 0.0;
+            if (has_prev) {
+#pragma unroll
+                for (int i0 = 0; i0 < 32; i0 += 8) {
+                    double mm[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) mm[k] = mq[i0 + k - 33];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) g = fma(-mm[k], g, halo[i0 + k]);
+                }
+            }
+#pragma unroll
+            for (int r0 = 0; r0 < 32; r0 += 8) {
+                double mm[8], bb[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { mm[k] = mq[r0 + k]; bb[k] = aq[r0 + k]; }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { g = fma(-mm[k], g, bb[k]); aq[r0 + k] = g; }
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 32; ++k) halo[k] = has_next ? aq[k + 33] : 0.0;
+        __syncthreads();
+        if (on) {
+            double sl = 0.0;
+            if (has_next) {
+#pragma unroll
+                for (int i0 = 24; i0 >= 0; i0 -= 8) {
+                    double cc[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) cc[k] = cq[i0 + k + 33];
+#pragma unroll
+                    for (int k = 7; k >= 0; --k) sl = fma(-cc[k], sl, halo[i0 + k]);
+                }
+            }
+#pragma unroll
+            for (int r0 = 31; r0 >= 0; r0 -= 8) {
+                double cc[8], gg[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { cc[k] = cq[r0 - k]; gg[k] = aq[r0 - k]; }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { sl = fma(-cc[k], sl, gg[k]); aq[r0 - k] = sl; }
+            }
+        }
+    } else {
+        // any other S: MBHL_SWEEP_BLOCKS blocks of ceil(S / MBHL_SWEEP_BLOCKS) rows per quantity, rows outside the matrix enter
+        // with coefficient 0
         // MBHL_SWEEP_BLOCKS blocks of rows per quantity: fewer blocks mean fewer redundant halo rows (instructions), more
         // blocks a shorter dependent chain
         constexpr int NB = MBHL_SWEEP_BLOCKS;
