@@ -63,6 +63,7 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
                 double* __restrict__ y_out) {
     extern __shared__ double sm[];
     __shared__ WalkerConst s_c;
+    __shared__ double s_cstar;
     const int SP = spline_sp(S), SY = spline_stride(S);
     double* xk = sm;                     // knots                                  [SP]
     double* ih = xk + SP;                // 1 / h_r, h_r = x_{r+1} - x_r          [SP]
@@ -101,6 +102,11 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
             xk[pad_idx(s)] = f;
             if (half == 0) knots[bm * S + s] = f;
         }
+        if (tid == 0) {
+            // fixed point of the pivot recurrence on an exactly geometric grid of ratio rho = exp(dlog): c = 1 / (2 (1 + rho) - rho c)
+            const double rho = exp(mc.dlog), b = 1.0 + rho;
+            s_cstar = (b - sqrt(b * b - rho)) / rho;
+        }
         __syncthreads();
         const int S0 = (S + 1) >> 1;
         const int s_lo = half ? S0 : 0, s_hi = half ? S : S0;
@@ -138,8 +144,12 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         const int m = (S + (int)kSplineThreads - 1) / (int)kSplineThreads;
         const int own0 = tid * m, own1 = min(S, own0 + m);
         if (own0 < own1) {
+            // The recurrence contracts by 0.07 per row towards the fixed point of the geometric grid, from which the true pivots
+            // differ by the rounding of the knots only (1e-13 relative): three rows from there are exact to fp64.  The first
+            // rows, where the not-a-knot row 0 is still felt, run the chain from row 0.
             double cp = 0.0;
-            int r = max(0, own0 - kSplineHaloPivot);
+            int r = 0;
+            if (own0 >= kSplineHaloPivot + 3) { r = own0 - 3; cp = s_cstar; }
             // three consecutive knots roll through registers: one shared-memory load per row
             double xa = (r > 0) ? xk[pad_idx(r - 1)] : 0.0, xb = xk[pad_idx(r)], xc = (r + 1 < S) ? xk[pad_idx(r + 1)] : 0.0;
             for (; r < own1; ++r) {
