@@ -195,13 +195,13 @@ __device__ inline double amp_hat(const WalkerConst& c, double f) {
     return v;
 }
 
-__device__ inline void psi_ins_raw(const WalkerConst& c, double f, double* psi, double* dpsi) {
+// v = cbrt(pi f), from the caller when it already has it (the mode amplitude of an inspiral knot needs the same cube root)
+__device__ inline void psi_ins_raw_v(const WalkerConst& c, double f, double v, double* psi, double* dpsi) {
     const double pf = kPi * f;
-    const double v = cbrt(pf);
     const double lnpf = log(pf);
-    const double invf = 1.0 / f;
     const double v2 = v * v, v3 = pf, v4 = v2 * v2, v5 = v4 * v, v6 = v3 * v3, v7 = v6 * v;
     const double iv5 = 1.0 / v5;
+    const double invf = kPi * (iv5 * v2);               // 1 / f = pi / v^3: one division fewer
     const double c5 = c.ph[5] * (1.0 + lnpf);
     const double c6 = c.ph[6] - (6848.0 / 63.0) * (kLn64 + lnpf);
     // series S = sum_i c_i v^i ; Psi_TF2 = -pi/4 + pre v^-5 S
@@ -213,6 +213,9 @@ __device__ inline void psi_ins_raw(const WalkerConst& c, double f, double* psi, 
     *psi = -0.25 * kPi + c.pre * iv5 * S +
            (c.sig[0] * f + 0.75 * c.sig[1] * f * f13 + 0.6 * c.sig[2] * f * f23 + 0.5 * c.sig[3] * f * f) * c.inveta;
     *dpsi = c.pre * iv5 * dS * invf + (c.sig[0] + c.sig[1] * f13 + c.sig[2] * f23 + c.sig[3] * f) * c.inveta;
+}
+__device__ inline void psi_ins_raw(const WalkerConst& c, double f, double* psi, double* dpsi) {
+    psi_ins_raw_v(c, f, cbrt(kPi * f), psi, dpsi);
 }
 
 __device__ inline void psi_int_raw(const WalkerConst& c, double f, double* psi, double* dpsi) {
@@ -304,10 +307,10 @@ __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_
     const double f = f_hz * c.M_s;
     const int m = c_mode_m[mi];
     // amplitude (O3): A_lm = amp0 * Ahat(f22A) * beta_lm(f)
+    const double V = cbrt(kTwoPi * f / m);
     {
         const int r = (f < mc.fiA) ? 0 : ((f < mc.fr) ? 1 : 2);
         const double f22 = mc.aA[r] * f + mc.bA[r];
-        const double V = cbrt(kTwoPi * f / m);
         double vp = 1.0;
         for (int i = 0; i < mc.vpow; ++i) vp *= V;
         const double beta = mc.ampc * vp / (V * V * V * sqrt(V));
@@ -317,7 +320,16 @@ __device__ inline void smooth_quantities(const WalkerConst& c, int mi, double f_
     double psi, dpsi;
     {
         const int r = (f < mc.fiP) ? 0 : ((f < mc.fr) ? 1 : 2);
-        psi22(c, mc.aP[r] * f + mc.bP[r], &psi, &dpsi);
+        const double f22 = mc.aP[r] * f + mc.bP[r];
+        if (r == 0 && f22 < kFPhiIns) {
+            // inspiral branch of the map: f22 = (2 / m) f, so cbrt(pi f22) is the V of the amplitude above
+            double p_, d_;
+            psi_ins_raw_v(c, f22, V, &p_, &d_);
+            psi = p_ - c.pshift - c.tshift * (f22 - c.f_ref);
+            dpsi = d_ - c.tshift;
+        } else {
+            psi22(c, f22, &psi, &dpsi);
+        }
         psi = psi * mc.invaP[r] + mc.cP[r];
     }
     const double t = c.t_coal + c.M_s * dpsi * (1.0 / kTwoPi);
