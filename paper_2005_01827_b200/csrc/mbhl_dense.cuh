@@ -25,8 +25,9 @@
 // One partial per (walker, CTA) leaves the kernel; k_final_reduce adds them in fixed order (bitwise
 // reproducible, no atomics on values).
 //
-// The loop body is FP64-pipe bound: per (bin, mode) 8 Horner cubics (24 DFMA), a quarter-turn sincos (17) and
-// 3 complex multiply-adds (12).  The linear term -2 pi f t_coal of the phase (reading G9) costs nothing here:
+// The loop body is bound by instruction issue (an FP64 instruction takes 2 cycles of a sub-partition, 3 with
+// three fresh register operands, and every other instruction 1): per (bin, mode) 8 Horner cubics (24 DFMA), a quarter-turn
+// sincos (14) and 3 complex multiply-adds (12).  The linear term -2 pi f t_coal of the phase (reading G9) costs nothing here:
 // k_spline folds it into the phase record of every interval (exact reduction of x_j t_coal, slope minus
 // t_coal), so the total phase of a bin in quarter turns is one cubic in u = f - x_j.
 #pragma once
