@@ -38,7 +38,7 @@ FLOP_PER_BIN = 40.0       # per (walker, active bin) epilo
 F_EVAL, F_EVAL_GATED, F_LANE, F_EPI = 98.0, 99.0, 105.0, 29.75
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_dense launch from the committed `ncu --set full` captures, by config
-DENSE_TRAFFIC = {2: (2.0444e9, "profiles/r02_dense_c2_ncu.txt (dram__bytes_read.sum 2.0350 GB + dram__bytes_write.sum 9.4 MB)")}
+DENSE_TRAFFIC = {2: (2.0385e9, "profiles/r02_dense_c2_ncu.txt (dram__bytes_read.sum 2.0289 GB + dram__bytes_write.sum 9.6 MB)")}
 
 
 def executed_flops(counts):
