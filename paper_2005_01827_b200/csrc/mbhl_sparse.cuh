@@ -9,13 +9,14 @@
 //   2. after one cluster barrier holds the S values of its 4 quantities and solves their slope systems as before:
 //      the matrix of a (walker, mode) is tridiagonal, strictly diagonally dominant and shared by the quantities.
 //      Every recurrence of the Thomas algorithm is contractive here (factors 0.07 for the pivots, 0.27 for both
-//      sweeps on log-spaced knots), so each is cut into blocks that start a few rows early from a zero state
-//      ("halo"): the influence of the cut is below fp64 rounding after 16 (pivots) / 32 (sweeps) rows, and blocks that
-//      reach row 0 / S-1 use the true not-a-knot rows.
+//      sweeps on log-spaced knots), so each is cut into blocks that start a few rows early ("halo"): the sweeps 32 rows
+//      early from a zero state (the influence of the cut is below fp64 rounding by then), the pivots 3 rows early from the
+//      fixed point of the recurrence on a geometric grid (the true pivots differ from it by the rounding of the knots
+//      only); blocks that reach row 0 / S-1 use the true not-a-knot rows.
 //        A. 1/h_r; pivots: thread t owns ceil(S/256) rows: c'_r = u_r / (d_r - a_r c'_{r-1}), 1 division per row
 //        B. b_r = rhs_r / (d_r - a_r c'_{r-1}) for 4 quantities, all rows in parallel
-//        C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of ceil(S/32) rows; operands of 8 steps
-//           are loaded before the 8 dependent multiply-adds)
+//        C. forward sweep g_r = b_r - m_r g_{r-1}   (warp = quantity, lane = block of 32 rows addressed with compile-time
+//           offsets when S is a multiple of 32 up to 1024; operands of 8 steps are loaded before the 8 dependent multiply-adds)
 //        D. backward sweep s_r = g_r - c'_r s_{r+1}
 //        E. c_j, d_j of every interval; each thread writes the 32 bytes of one (interval, quantity) with ONE 256-bit
 //           store, a warp 8 full 128-byte lines.
