@@ -215,6 +215,7 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
     __shared__ DenseWalker s_dw[kMaxW];
     __shared__ double s_xj[kRecSlots];                              // knot x_j of each staged record
     __shared__ PairDesc s_desc[kPairs];
+    __shared__ unsigned s_cls[kPairs];                              // per pair: 8 class bits for each of the CTA's warp tiles (prepare step)
     __shared__ double s_acc[kDenseThreads / 32][kMaxW][2];
     __shared__ __align__(8) unsigned long long s_bar;
     __shared__ int s_range[2];
@@ -312,6 +313,25 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
                 }
             }
             s_desc[tid] = d;
+            // class of the pair in each warp tile: 1 = the whole tile lies in the segment served by slot 2p, 2 = by slot 2p + 1,
+            // 4 = partly covered (knot or band edge inside the tile), 8 = three or more intervals in the chunk (general path)
+            unsigned cw = 0;
+#pragma unroll
+            for (int w = 0; w < kDenseThreads / 32; ++w) {
+                const int t0 = w * kWarpTile, t1 = t0 + kWarpTile - 1;
+                unsigned c = 0;
+                if (d.kind == 1) {
+                    const int loA = max((int)d.a, t0), hiA = min((int)d.ks - 1, t1);
+                    const int loB = max((int)d.ks, t0), hiB = min((int)d.b, t1);
+                    if (loA == t0 && hiA == t1) c = 1u;
+                    else if (loB == t0 && hiB == t1) c = 2u;
+                    else if (loA <= hiA || loB <= hiB) c = 4u;
+                } else if (d.kind == 2) {
+                    if (max((int)d.a, t0) <= min((int)d.b, t1)) c = 8u;
+                }
+                cw |= c << (8 * w);
+            }
+            s_cls[tid] = cw;
         }
         cp_async_wait_all();
         __syncthreads();
@@ -325,24 +345,13 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
         for (int r = 0; r < kDenseR; ++r) f[r] = sf[lane + 32 * r];
 
         for (int wi = 0; wi < nb; ++wi) {
-            // lanes 0..5 classify mode `lane` for this warp tile: segment A = bins served by slot 2p, B = by slot 2p+1
-            int loA = 1, hiA = 0, loB = 1, hiB = 0;
-            bool fullA = false, fullB = false, part = false, gen = false;
-            if (lane < MBHL_NMODE) {
-                const PairDesc d = s_desc[wi * MBHL_NMODE + lane];
-                if (d.kind == 1) {
-                    loA = max((int)d.a, t0); hiA = min((int)d.ks - 1, t1);
-                    loB = max((int)d.ks, t0); hiB = min((int)d.b, t1);
-                    fullA = loA == t0 && hiA == t1;
-                    fullB = loB == t0 && hiB == t1;
-                    part = !fullA && !fullB && (loA <= hiA || loB <= hiB);
-                } else if (d.kind == 2) {
-                    gen = max((int)d.a, t0) <= min((int)d.b, t1);
-                }
-            }
-            unsigned m_full = __ballot_sync(0xffffffffu, fullA || fullB);
-            const unsigned m_selB = __ballot_sync(0xffffffffu, fullB);
-            unsigned m_part = __ballot_sync(0xffffffffu, part);
+            // lanes 0..5 read the class of mode `lane` in this warp tile (set by the prepare step)
+            unsigned cls = 0;
+            if (lane < MBHL_NMODE) cls = (s_cls[wi * MBHL_NMODE + lane] >> (8 * warp)) & 0xffu;
+            const bool gen = (cls & 8u) != 0;
+            unsigned m_full = __ballot_sync(0xffffffffu, (cls & 3u) != 0);
+            const unsigned m_selB = __ballot_sync(0xffffffffu, (cls & 2u) != 0);
+            unsigned m_part = __ballot_sync(0xffffffffu, (cls & 4u) != 0);
             unsigned m_gen = __ballot_sync(0xffffffffu, gen);
             if (!(m_full | m_part | m_gen)) continue;
 
@@ -362,8 +371,9 @@ __global__ void __launch_bounds__(kDenseThreads, MBHL_DENSE_MINB) k_dense(DenseA
             while (m_part) {
                                 const int mi = __ffs(m_part) - 1;
                 m_part &= m_part - 1;
-                const int lo0 = __shfl_sync(0xffffffffu, loA, mi), hi0 = __shfl_sync(0xffffffffu, hiA, mi);
-                const int lo1 = __shfl_sync(0xffffffffu, loB, mi), hi1 = __shfl_sync(0xffffffffu, hiB, mi);
+                const PairDesc d = s_desc[wi * MBHL_NMODE + mi];
+                const int lo0 = max((int)d.a, t0), hi0 = min((int)d.ks - 1, t1);     // segment served by slot 2p
+                const int lo1 = max((int)d.ks, t0), hi1 = min((int)d.b, t1);         // segment served by slot 2p + 1
                 const int slot0 = 2 * (wi * MBHL_NMODE + mi);
                 if (lo0 <= hi0 && lo1 <= hi1) {
                     // a knot inside the warp tile: every bin reads the staged record of its own side, one pass
