@@ -385,6 +385,22 @@ def test_tiny_grids_and_few_knots(table, cfg0):
         M.mbhl_free(ctx)
 
 
+def test_many_knots_up_to_the_documented_ceiling(table, cfg0):
+    # S above 1024 (up to the ceiling mbhl.h documents, 2048): the sweeps of the fused sparse kernel leave their 32-row fast
+    # path, a CTA's shared memory holds twice the rows; S = 1056 is the first multiple of 32 beyond the fast path
+    sl = slice(1000, 9000)
+    f, d, s_ = cfg0["freqs"][sl].copy(), np.ascontiguousarray(cfg0["data"][:, sl]), np.ascontiguousarray(cfg0["psd"][:, sl])
+    p = cfg0["params"][:2]
+    for S in (1056, 1536, 2048):
+        ctx = M.mbhl_init(dev(f), dev(d), dev(s_), sparse_points=S)
+        dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(p))]
+        for b in range(2):
+            rdh, rhh, rll = L.loglike_parts(table, p[b], f, d, s_, S, 0.0)
+            assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (S, b, ll[b], rll)
+            assert abs(hh[b] - rhh) <= 1e-8 * max(rhh, 1e-300), (S, b, hh[b], rhh)
+        M.mbhl_free(ctx)
+
+
 def test_narrow_interval_regime_random_masses(table):
     # BASELINE config 4 corner: few bins per spline interval (N = 2^14 bins up to 0.1 Hz with S = 1024 knots) and walkers
     # from 1e5 to 1e8 solar masses in one batch: every path of the dense kernel (staged, knot straddles, scratch, per bin)
