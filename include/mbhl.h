@@ -146,6 +146,31 @@ int mbhl_loglike_sampled(mbhl_ctx* ctx, const double* theta, int64_t B, double* 
  * walker outside the prior box).  Testing aid; asynchronous on the context's stream.                                    */
 int mbhl_unpack_coords(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* params_out);
 
+/* mbhl_unpack_coords for callers that must not allocate device memory.
+ * WHO THAT IS: mbhl_unpack_coords (like every hot-path call) takes its per-walker records from the context's workspace,
+ * and on a context created without max_batch or a caller workspace that means a cudaMalloc inside the call.  Some callers
+ * cannot afford or are not allowed that: a sampler sharing the GPU with a framework whose memory pool has already claimed
+ * all free HBM (the cudaMalloc would simply fail), a job running under a fixed per-process memory quota, or a latency-critical
+ * loop in which cudaMalloc / cudaFree would stall the device's other streams while they run.  For them this entry point does the same
+ * conversion - the same kernel, k_walker_consts - with the kernel's scratch records (the WalkerConst and DenseWalker of every
+ * row, about 2.5 KB per walker, which this call computes and then discards) placed in a fixed array that is part of the
+ * library image instead of in allocated memory.  It calls no cudaMalloc, cudaFree or any allocating library routine.
+ *   rows[B][11] (device, in `coords`) -> params_out[B][11] (device): physical SSB parameters, a NaN row for a walker outside
+ *   the prior box - bit-for-bit what mbhl_unpack_coords writes.  Caller owns both; they must not overlap (MBHL_EINVAL).
+ * LIMIT: B <= MBHL_STATIC_MAX_WALKERS per call; a larger B is refused with MBHL_EINVAL and a message naming the limit
+ * (split the batch).  The array is sized for exactly that many walkers (about 2.6 MB) and every GPU on which the library
+ * is loaded holds it until the process exits, whether or not this call is ever made.
+ * FIRST CALL: the first call on each device looks up the array's device address (cudaGetSymbolAddress, once per device,
+ * kept for the process's lifetime); that lookup may make the driver load the library's module.  Make this first call
+ * during set-up, before any stream capture is begun.
+ * SHARING: there is ONE array per device, shared by every context, stream and thread, and it keeps the previous call's
+ * records.  Nothing in it has to start at zero - each call overwrites the records of its rows 0..B-1 before anything could
+ * read them and never looks at the rest - so stale contents are harmless.  But two calls whose kernels can overlap on the
+ * same GPU (different streams, different contexts, different host threads) write the same records and race: keep calls on one
+ * device ordered on one stream, or synchronise between them.  Asynchronous on the context's stream.                      */
+#define MBHL_STATIC_MAX_WALKERS 1024
+int mbhl_unpack_coords_static(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* params_out);
+
 /* Parallel-tempered affine-invariant ensemble: n_temps rungs with inverse temperatures
  * betas[t] (host pointer; beta = 0 is T = infinity, :222), n_walkers (even) walkers per rung in the sampler's
  * coordinates, theta0[n_temps][n_walkers][11] (host or device pointer, copied).  One step = for each half of the

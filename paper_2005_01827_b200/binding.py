@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmbhl.so")
 NPARAM, NMODE, NQ = 11, 6, 8
 COORDS_PHYSICAL, COORDS_SAMPLED, COORDS_SAMPLED_LISA = 0, 1, 2        # include/mbhl.h MBHL_COORDS_*
-SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free", "mbhl_het_init", "mbhl_het_loglike", "mbhl_het_free",
+SYMBOLS = ("mbhl_noise", "mbhl_mode_products", "mbhl_loglike_sampled", "mbhl_loglike_coords", "mbhl_unpack_coords", "mbhl_unpack_coords_static", "mbhl_pt_init", "mbhl_pt_step", "mbhl_pt_state", "mbhl_pt_free", "mbhl_het_init", "mbhl_het_loglike", "mbhl_het_free",
            "mbhl_init", "mbhl_loglike", "mbhl_loglike_parts", "mbhl_loglike_host", "mbhl_template", "mbhl_sparse",
            "mbhl_workspace_bytes", "mbhl_set_workspace", "mbhl_data_norm", "mbhl_num_bins", "mbhl_sparse_points",
            "mbhl_launch_count", "mbhl_last_work", "mbhl_last_dense_work", "mbhl_enable_stage_timing", "mbhl_stage_times", "mbhl_dfma_probe", "mbhl_strerror", "mbhl_last_error", "mbhl_free")
@@ -50,6 +50,7 @@ def lib():
         L.mbhl_loglike_sampled.argtypes = [vp, vp, i64, vp]
         L.mbhl_loglike_coords.argtypes = [vp, vp, i64, i32, vp]
         L.mbhl_unpack_coords.argtypes = [vp, vp, i64, i32, vp]
+        L.mbhl_unpack_coords_static.argtypes = [vp, vp, i64, i32, vp]
         L.mbhl_pt_init.argtypes = [vp, ctypes.POINTER(vp), vp, vp, i32, i32, ctypes.c_uint64, dbl, i32]
         L.mbhl_pt_step.argtypes = [vp, i32]
         L.mbhl_pt_state.argtypes = [vp, vp, vp, vp, vp]
@@ -244,6 +245,22 @@ def mbhl_unpack_coords(ctx, rows, coords):
     B = int(rows.shape[0])
     out = torch.empty((B, NPARAM), dtype=torch.float64, device=rows.device)
     _check(lib().mbhl_unpack_coords(ctx, _ptr(rows), B, int(coords), _ptr(out)), ctx)
+    return out
+
+
+STATIC_MAX_WALKERS = 1024            # include/mbhl.h MBHL_STATIC_MAX_WALKERS
+
+
+def mbhl_unpack_coords_static(ctx, rows, coords, out):
+    """mbhl_unpack_coords for callers that must not allocate device memory (a memory pool already owns the GPU's free
+    HBM, a fixed memory quota, a loop that cannot take cudaMalloc's stall): the kernel's scratch records live in a fixed
+    array of the library, so the C call allocates nothing - and neither does this wrapper, which is why `out` [B, 11]
+    (float64, CUDA, not overlapping `rows`) is passed in instead of created here.  At most STATIC_MAX_WALKERS rows per
+    call (MbhlError above that).  Make the first call on a device during set-up; calls that can overlap on one GPU race
+    on the shared array (include/mbhl.h has the full rules).  Returns `out`."""
+    B = int(rows.shape[0])
+    assert tuple(out.shape) == (B, NPARAM)
+    _check(lib().mbhl_unpack_coords_static(ctx, _ptr(rows), B, int(coords), _ptr(out)), ctx)
     return out
 
 

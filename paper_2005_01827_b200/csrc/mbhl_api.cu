@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -869,6 +870,81 @@ int mbhl_stage_times(mbhl_ctx* ctx, double ms[5]) {
             ms[i] += (double)t / n;
         }
     ctx->n_timed = 0;
+    return MBHL_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// mbhl_unpack_coords_static: the coordinate conversion with the kernel's scratch records in a fixed array of the
+// library image, for callers that must not allocate device memory (who they are and the rules: include/mbhl.h)
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t kStaticConstsBytes = up256((size_t)MBHL_STATIC_MAX_WALKERS * sizeof(WalkerConst));
+constexpr size_t kStaticDenseBytes = up256((size_t)MBHL_STATIC_MAX_WALKERS * sizeof(DenseWalker));
+constexpr size_t kStaticScratchBytes = kStaticConstsBytes + kStaticDenseBytes;      // about 2.6 MB
+static_assert(kStaticScratchBytes <= ((size_t)4 << 20), "the fixed scratch array is meant to stay small: every GPU holds it until exit");
+
+// [WalkerConst x MBHL_STATIC_MAX_WALKERS][DenseWalker x MBHL_STATIC_MAX_WALKERS], written by k_walker_consts and read by
+// nobody.  One copy per device that loads the library, for the process's lifetime.  NOTE for host code: this NAME is only
+// a host-side stand-in for the symbol, not a device address - a kernel handed `g_static_scratch` itself would fault (or,
+// where the GPU can reach host memory, quietly use the wrong memory).  Host code must go through static_scratch_base().
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_base[kStaticMaxDevices] = {};      // device address of g_static_scratch, per device ordinal; looked up once
+
+// Device address of the array on ctx->device, which must be the current device.  The first call per device asks the
+// runtime (cudaGetSymbolAddress resolves the symbol in the CURRENT device's copy of the module); later calls reuse it.
+int static_scratch_base(mbhl_ctx* ctx, char** base) {
+    const int d = ctx->device;
+    if (d < 0 || d >= kStaticMaxDevices) return fail(ctx, MBHL_EINVAL, "mbhl_unpack_coords_static: device ordinal outside 0..63");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_base[d]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_static_scratch);
+        if (e != cudaSuccess) return fail(ctx, MBHL_ECUDA, "cudaGetSymbolAddress(g_static_scratch)", e);
+        if (!ptr) return fail(ctx, MBHL_ECUDA, "cudaGetSymbolAddress(g_static_scratch) returned a null address");
+        g_static_base[d] = ptr;
+    }
+    *base = (char*)g_static_base[d];
+    return MBHL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mbhl_unpack_coords_static(mbhl_ctx* ctx, const double* rows, int64_t B, int32_t coords, double* params_out) {
+    if (!ctx) return MBHL_EINVAL;
+    if (B < 0 || (B > 0 && (!rows || !params_out)) || coords < 0 || coords > 2)
+        return fail(ctx, MBHL_EINVAL, "mbhl_unpack_coords_static: bad rows/B/coords/params_out");
+    if (B > MBHL_STATIC_MAX_WALKERS) {
+        snprintf(ctx->err, sizeof(ctx->err),
+                 "mbhl_unpack_coords_static: B = %lld exceeds MBHL_STATIC_MAX_WALKERS = %d, the size of the fixed scratch array; split the batch",
+                 (long long)B, MBHL_STATIC_MAX_WALKERS);
+        return MBHL_EINVAL;
+    }
+    if (B == 0) return MBHL_OK;
+    {
+        // the kernel reads rows and writes params_out through __restrict__ pointers: the two may not share memory
+        const uintptr_t r0 = (uintptr_t)rows, p0 = (uintptr_t)params_out, n = (uintptr_t)B * MBHL_NPARAM * sizeof(double);
+        if (r0 < p0 + n && p0 < r0 + n) return fail(ctx, MBHL_EINVAL, "mbhl_unpack_coords_static: rows and params_out overlap");
+    }
+    CU(cudaSetDevice(ctx->device));
+    char* base = nullptr;
+    const int rc = static_scratch_base(ctx, &base);
+    if (rc != MBHL_OK) return rc;
+    // Same launch as run_consts(), with the two record arrays in the fixed array and the converted parameters going
+    // straight to the caller's buffer.  Rows 0..B-1 of both record arrays are overwritten in full; nothing is read back.
+    k_walker_consts<<<(unsigned)((B + kConstsWarps - 1) / kConstsWarps), 32 * kConstsWarps, 0, ctx->stream>>>(
+        rows, B, coords, ctx->t0, ctx->f_min, ctx->f_max, ctx->S, ctx->mode_mask, ctx->freqs, (int)ctx->N, ctx->df,
+        (WalkerConst*)base, (DenseWalker*)(base + kStaticConstsBytes), params_out);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
     return MBHL_OK;
 }
 
