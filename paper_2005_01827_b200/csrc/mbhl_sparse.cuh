@@ -94,6 +94,11 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
             for (int i = tid; i < kSplineQ * S; i += kSplineThreads) y_out[(bm * MBHL_NQ + half * kSplineQ) * S + i] = 0.0;
         return;
     }
+    // The evaluation loop below stores into the PEER CTA's shared memory.  Distributed shared memory may only be touched once
+    // the peer is known to have started: arrive here, wait just before the first remote store, with the knot set-up in between
+    // to cover the latency.  (The `!active` return above is taken by both CTAs of a pair or by neither, so the pair always
+    // agrees on whether this barrier exists.)
+    cluster.barrier_arrive();
     const double t_coal = c.t_coal;
     // 1. knots (both CTAs, identical arithmetic), then the smooth functions at this CTA's half of them
     {
@@ -112,6 +117,7 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
         const int S0 = (S + 1) >> 1;
         const int s_lo = half ? S0 : 0, s_hi = half ? S : S0;
         double* Ypeer = cluster.map_shared_rank(Y, half ^ 1);
+        cluster.barrier_wait();                          // the peer CTA is running: its shared memory exists
         for (int s = s_lo + tid; s < s_hi; s += kSplineThreads) {
             double q[MBHL_NQ];
             smooth_quantities(c, mi, xk[pad_idx(s)], q);
