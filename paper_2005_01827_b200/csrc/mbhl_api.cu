@@ -152,6 +152,8 @@ bool is_device_ptr(const void* p) {
 // running maximum so that contexts with different S can coexist (several contexts may be alive at once, mbhl.h).
 int ensure_spline_smem(mbhl_ctx* ctx) {
     static size_t granted[64] = {0};
+    static std::mutex mu;                                // contexts on different host threads share this table
+    std::lock_guard<std::mutex> lock(mu);
     const size_t need = spline_smem_bytes(ctx->S);
     const int d = ctx->device & 63;
     if (granted[d] < need) {
@@ -930,7 +932,8 @@ int mbhl_unpack_coords_static(mbhl_ctx* ctx, const double* rows, int64_t B, int3
     }
     if (B == 0) return MBHL_OK;
     {
-        // the kernel reads rows and writes params_out through __restrict__ pointers: the two may not share memory
+        // a warp writes its converted row while other warps may still be reading theirs: fine for distinct buffers (and for
+        // the exactly-in-place use inside the library), wrong for buffers that overlap at an offset - refuse any overlap
         const uintptr_t r0 = (uintptr_t)rows, p0 = (uintptr_t)params_out, n = (uintptr_t)B * MBHL_NPARAM * sizeof(double);
         if (r0 < p0 + n && p0 < r0 + n) return fail(ctx, MBHL_EINVAL, "mbhl_unpack_coords_static: rows and params_out overlap");
     }

@@ -120,10 +120,12 @@ constexpr int kConstsWarps = 4;      // walkers per CTA of k_walker_consts (one 
 // sampler's coordinates with (lambda, sin beta, psi, ln t) in the LISA frame (reading G20).  The
 // conversion runs in registers here, so a sampler hands over raw walker coordinates and no extra kernel runs.
 // params_out (may be null): the physical SSB parameters the walker was converted to (NaN row if outside the box).
-__global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const double* __restrict__ rows, int64_t B, int coords, double t0, double f_min,
+// rows and params_out carry no __restrict__: mbhl_loglike_host hands over the same buffer for both (a warp reads its own
+// row in full, then writes it back after the __syncwarp below; no other warp touches that row).
+__global__ void __launch_bounds__(32 * kConstsWarps) k_walker_consts(const double* rows, int64_t B, int coords, double t0, double f_min,
                                                       double f_max, int S, uint32_t mode_mask, const double* __restrict__ freqs,
                                                       int N, double df, WalkerConst* __restrict__ out,
-                                                      DenseWalker* __restrict__ dw, double* __restrict__ params_out) {
+                                                      DenseWalker* __restrict__ dw, double* params_out) {
     __shared__ WalkerConst s_c[kConstsWarps];
     __shared__ DenseWalker s_d[kConstsWarps];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
