@@ -201,7 +201,7 @@ void mbhl_pt_free(mbhl_pt* pt);
  * mbhl_het_loglike then evaluates walkers from the summary data: per walker the sparse stage (a1-a5) plus
  * 3 n_coarse spline evaluations per mode, instead of one per fine bin.  The envelope A That exp(i (theta - theta_ref))
  * is taken piecewise parabolic on the coarse bins (values at a bin's first, centre and last frequency): exact for one
- * fine bin per coarse bin, third order in the coarse bin width otherwise, accurate for walkers whose phase stays within a fraction of a cycle of the reference's across a
+ * fine bin per coarse bin; otherwise the error of the sums falls at least with the cube of the coarse bin width (with its fourth power on bins that hold no band edge and no region boundary of the model: pinned on the oracle in tests/test_oracle_heterodyne.py); accurate for walkers whose phase stays within a fraction of a cycle of the reference's across a
  * coarse bin (the bulk of a posterior).  The band of a mode is taken to be the reference's; no spline is extrapolated.  d_h, h_h, logL [B]: device
  * pointers, any may be NULL; asynchronous on the context's stream.  The context must outlive the handle.            */
 typedef struct mbhl_het mbhl_het;

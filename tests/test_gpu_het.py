@@ -80,6 +80,7 @@ def test_het_config2_scale_parity_and_accuracy(table):
         # the reference (b = 0) cancels exactly on both sides
         tol = 1e-8 if b == 0 else 3e-7
         assert abs(hh[b] - rhh) <= tol * rhh and abs(dh[b] - rdh) <= tol * max(abs(rdh), rhh), (b, dh[b], rdh, hh[b], rhh)
+        assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (b, ll[b], rll)          # the north_star bar on logL itself
     # accuracy against the brute-force path: a small fraction of <h|h>, shrinking with more coarse bins
     err512 = np.max(np.abs(hh - bhh) / bhh)
     het2 = M.mbhl_het_init(ctx, dev(inj), W.het_edges(freqs, 2048, f_lo, f_hi))

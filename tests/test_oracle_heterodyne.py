@@ -62,3 +62,37 @@ def test_edges_generator_and_degenerate_inputs(table):
     heavy[0] = 1e10                                   # every band below the grid: no signal
     dh, hh, ll = H.loglike_parts(table, summ, heavy)
     assert dh == 0.0 and hh == 0.0 and ll == -0.5 * summ["dd"]
+
+
+def test_order_of_convergence_on_a_window_without_band_edges_or_model_kinks(table):
+    # What mbhl.h promises for mbhl_het_*: the error falls at least with the CUBE of the coarse bin width.  A parabola through
+    # three points of a smooth envelope leaves an error r''' x (x^2 - s^2) / 6, odd about the bin centre, whose sum against
+    # slowly varying weights cancels to leading order - so on clean bins the sums converge with the FOURTH power (a factor 16
+    # per halving).  The window is chosen so that nothing else contributes: 0.3-1.2 mHz for a 1e6 Msun binary 2e7 s before
+    # merger lies inside the band of all six modes (every f_lo is below the window, every f_hi above) and inside the inspiral
+    # region of every mode's amplitude and phase maps ((2,1): M f < 0.007), the data are the noise-free injection, and the
+    # walker sits 1e-4 (relative) away from the reference so that the errors stay far above rounding.  Dropping the
+    # second-order moments (A2, B2) or mis-centring the parabola turns this into second-order convergence (a factor 4).
+    n = 4096
+    freqs = np.linspace(3e-4, 1.2e-3, n)
+    psd = W.scird_psd_aet(freqs)
+    S = 128
+    inj = np.array([1e6, 3.0, 0.6, -0.3, 10.0, 1.3, 0.9, 2.1, 0.4, 0.7, 2.0e7])
+    for mo in L.sparse_stage(table, inj, freqs[0], freqs[-1], S, 0.0)[0]:
+        assert mo is not None and mo["knots"][0] == freqs[0] and mo["knots"][-1] == freqs[-1]     # in band throughout
+    data = L.template(table, inj, freqs, S)
+    walker = W.perturb(np.random.default_rng(5), inj, 1, 1e-4)[0]
+    rdh, rhh, _ = L.loglike_parts(table, walker, freqs, data, psd, S)
+    e_hh, e_dh = [], []
+    for nb in (8, 16, 32, 64):
+        edges = np.unique(np.round(np.linspace(0, n, nb + 1)).astype(np.int64))
+        summ = H.setup(table, inj, freqs, data, psd, S, edges)
+        assert summ["edges"].size == nb + 1                                                       # no band edge refined the bins
+        dh, hh, _ = H.loglike_parts(table, summ, walker)
+        e_hh.append(abs(hh - rhh) / rhh)
+        e_dh.append(abs(dh - rdh) / rhh)
+    for a, b in ((0, 1), (1, 2)):
+        assert 10.0 < e_hh[a] / e_hh[b] < 24.0, e_hh          # fourth order: 16 per halving
+        assert e_dh[a] / e_dh[b] > 8.0, e_dh                   # at least third
+    assert e_hh[0] / e_hh[3] > 512.0 and e_dh[0] / e_dh[3] > 512.0, (e_hh, e_dh)      # at least the cube over three halvings
+    assert e_hh[0] < 1e-3 and e_hh[3] < 1e-6

@@ -140,3 +140,96 @@ def test_higher_mode_table_rows_follow_from_the_leading_pn_multipoles(table):
         assert abs(table[f"hm.{l}{m}.amp"] - c) < 1e-15, (l, m)
         d = table[f"hm.{l}{m}.dphi"] - dphi
         assert abs(d - 2 * math.pi * round(d / (2 * math.pi))) < 1e-14, (l, m)
+
+
+def _newtonian_chirp_spectrum(eta, delta, l, m, dt=1.0, n=1 << 20):
+    """|FFT| of the leading-PN time-domain multipole h_{l,-m}(t) = (-1)^l conj(h_lm) of a Newtonian quasi-circular inspiral
+    (geometric units, M = 1, R = 1):  h_lm = 2 eta x sqrt(16 pi/5) H_lm(x) exp(-i m phi),  x = (omega_orb)^(2/3),
+    Theta = eta (t_c - t)/5,  x = Theta^(-1/4)/4,  phi = -Theta^(5/8)/eta  (textbook, Blanchet's review / Kidder 2008).
+    H_lm with their mass factors and powers of x are typed here from that literature, independently of oracle/phenom.py.
+    The record runs from orbital M omega = 0.004 to 0.055 with a smooth taper over 0.004-0.006 and 0.040-0.055, zero-padded
+    to n samples.  Returns (f [cycles per M], |h~(f)|) on the FFT grid."""
+    s = math.sqrt
+    tau = lambda om: 5.0 / (256.0 * eta) * om ** (-8.0 / 3.0)          # time to coalescence at orbital frequency om
+    t = np.arange(-tau(0.004), -tau(0.055), dt)                        # t_c = 0
+    assert t.size < n
+    theta = eta * (-t) / 5.0
+    x = 0.25 * theta ** -0.25
+    om = x ** 1.5
+    phi = -theta ** 0.625 / eta
+    H = {(2, 2): 1.0 + 0.0 * x,
+         (2, 1): -1j / 3.0 * delta * x ** 0.5,
+         (3, 3): -0.75j * s(15.0 / 14.0) * delta * x ** 0.5,
+         (3, 2): s(5.0 / 7.0) / 3.0 * (1.0 - 3.0 * eta) * x,
+         (4, 4): -8.0 / 9.0 * s(5.0 / 7.0) * (1.0 - 3.0 * eta) * x,
+         (4, 3): -9j / (4.0 * s(70.0)) * delta * (1.0 - 2.0 * eta) * x ** 1.5}[(l, m)]
+    h = 2.0 * eta * x * s(16.0 * math.pi / 5.0) * H * np.exp(-1j * m * phi)
+    h = (-1.0) ** l * np.conj(h)                           # h_{l,-m}: the positive-frequency content (reading G3)
+
+    def ramp(u):                                           # C-infinity step from 0 (u <= 0) to 1 (u >= 1)
+        u = np.clip(u, 2e-3, 1.0 - 2e-3)
+        return 1.0 / (1.0 + np.exp(1.0 / u - 1.0 / (1.0 - u)))
+    w = ramp((t + tau(0.004)) / (tau(0.004) - tau(0.006))) * ramp((-tau(0.055) - t) / (tau(0.040) - tau(0.055)))
+    spec = np.fft.fft(h * w, n) * dt
+    return np.fft.fftfreq(n, dt), np.abs(spec)
+
+
+@pytest.mark.parametrize("q", [3.0, 5.0, 1.5])
+def test_beta_lm_structure_against_the_fft_of_a_newtonian_chirp(table, q):
+    # Pins WHICH mass factor (delta, 1 - 3 eta, delta (1 - 2 eta)) and WHICH power of V every mode amplitude carries in
+    # Intrinsic.beta_lm, and its V^(-7/2) sqrt(2/m) stationary-phase prefactor: the FFT of the time-domain leading-PN
+    # multipole of a Newtonian chirp, divided by the (2,2) spectrum at the same orbital frequency, must equal
+    # beta_lm(f) / beta_22(2 f / m).  Three mass ratios so that delta, (1 - 3 eta) and (1 - 2 eta) all move; several orbital
+    # frequencies so that a wrong power of V shows as a slope.  Measured agreement is ~1e-3 (stationary phase: omega_dot /
+    # omega^2 ~ 1e-3 here, plus taper ripple); the bar is 1 %.
+    I = Intrinsic(table, 1e6, q, 0.0, 0.0, 10.0)
+    eta, delta = I.eta, I.delta
+    f22, s22 = _newtonian_chirp_spectrum(eta, delta, 2, 2)
+    pos = f22 > 0
+    for (l, m) in MODES:
+        # orbital M omega: V = omega^(1/3) = 0.20 ... 0.27, a factor 1.36 in V, so one power of V off is a 36 % slope.  The m = 1
+        # mode has half the cycles of (2,2) at a given orbital frequency and its taper ripple passes 1 % above 0.015
+        omegas = np.array([0.008, 0.011, 0.015, 0.020]) if m > 1 else np.array([0.008, 0.011, 0.015])
+        flm, slm = _newtonian_chirp_spectrum(eta, delta, l, m)
+        f_m = m * omegas / (2.0 * math.pi)
+        f_2 = 2.0 * omegas / (2.0 * math.pi)
+        got_lm = np.interp(f_m, flm[pos], slm[pos])
+        got_22 = np.interp(f_2, f22[pos], s22[pos])
+        # absolute level of every mode against the oracle's formula (1 %: stationary phase + taper ripple)
+        want = I.beta_lm(l, m, f_m)
+        assert np.max(np.abs(got_lm / want - 1.0)) < 1e-2, ((l, m), got_lm / want)
+        # ratio to (2,2) at the same orbital frequency: what amp_lm multiplies A_22 by in the inspiral
+        ratio_fft = got_lm / got_22
+        ratio_oracle = I.beta_lm(l, m, f_m) / I.beta_lm(2, 2, f_2)
+        assert np.max(np.abs(ratio_fft / ratio_oracle - 1.0)) < 1e-2, ((l, m), ratio_fft / ratio_oracle)
+
+
+@pytest.mark.parametrize("M,q,a1,a2", CASES[:4])
+def test_ringdown_amplitude_of_every_mode_is_the_22_lorentzian_shifted_to_its_own_f_rd(table, M, q, a1, a2):
+    # SURVEY 8(c) O3: in the ringdown region the amplitude map is the SHIFT f_22 = f - (f_RD,lm - f_RD,22), slope one (the phase
+    # map has slope f_damp,22 / f_damp,lm instead).  Stated without the map: with R_lm(f) = A_lm(f) / beta_lm(f), the leading-PN
+    # factor stripped, R_lm(f_RD,lm + x) = R_22(f_RD,22 + x) for x >= 0, so the Lorentzian of every mode peaks at the same offset
+    # from its own ringdown frequency and has the (2,2) width.  A slope other than one changes the measured half-width below.
+    I = Intrinsic(table, M, q, a1, a2, 10.0)
+    R = lambda l, m, f: I.amp_lm(l, m, np.float64(f)) / I.beta_lm(l, m, np.float64(f))
+    w22 = I.gamma3 * I.fDM
+
+    def half_width(l, m):
+        # x > 0 with R(f_RD + x) = R(f_RD) / 2, by bisection on the measured curve
+        f0 = I.f_rd[(l, m)]
+        r0 = R(l, m, f0)
+        lo, hi = 0.0, 20.0 * w22
+        assert R(l, m, f0 + hi) < 0.5 * r0
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            lo, hi = (mid, hi) if R(l, m, f0 + mid) > 0.5 * r0 else (lo, mid)
+        return 0.5 * (lo + hi)
+
+    hw22 = half_width(2, 2)
+    assert 0.2 * w22 < hw22 < 3.0 * w22                    # of the order of the Lorentzian's width gamma3 f_damp,22
+    for (l, m) in MODES[1:]:
+        if I.beta_lm(l, m, np.float64(0.1)) == 0.0:
+            continue                                       # odd-m modes of an equal-mass binary vanish
+        for x in (0.0, 0.3 * w22, w22, 4.0 * w22):
+            assert R(l, m, I.f_rd[(l, m)] + x) == pytest.approx(R(2, 2, I.fRD + x), rel=1e-11), ((l, m), x)
+        assert half_width(l, m) == pytest.approx(hw22, rel=1e-9), (l, m)
