@@ -58,17 +58,16 @@ def edge_mask(table, params, freqs, t0):
     return mask
 
 
-def test_sparse_stage_parity(table, cfg0):
-    ctx = make_ctx(cfg0)
-    params = cfg0["params"]
-    knots, y, coef = [t.cpu().numpy() for t in M.mbhl_sparse(ctx, dev(params))]
-    S = cfg0["S"]
+def check_sparse_stage(table, params, knots, y, coef, f_lo, f_hi, S, t0):
+    """Element-by-element comparison of mbhl_sparse's three outputs with the oracle's sparse stage; returns the number of active modes."""
+    n_active = 0
     for b in range(params.shape[0]):
-        modes, _ = L.sparse_stage(table, params[b], cfg0["freqs"][0], cfg0["freqs"][-1], S, cfg0["t0"])
+        modes, _ = L.sparse_stage(table, params[b], f_lo, f_hi, S, t0)
         for mi, mo in enumerate(modes):
             if mo is None:
                 assert np.all(knots[b, mi] == 0.0) and np.all(coef[b, mi] == 0.0)
                 continue
+            n_active += 1
             assert np.max(np.abs(knots[b, mi] / mo["knots"] - 1.0)) < 1e-13
             yo = mo["y"]
             amp_scale = np.max(np.abs(yo[0]))
@@ -93,6 +92,34 @@ def test_sparse_stage_parity(table, cfg0):
                         d = d - np.rint(d)
                         assert np.max(np.abs(cg[:, q, col])) <= 0.5 + 1e-12
                     assert np.max(np.abs(d)) <= tol, (b, mi, q, col, np.max(np.abs(d)), tol)
+    return n_active
+
+
+def test_sparse_stage_parity(table, cfg0):
+    ctx = make_ctx(cfg0)
+    params = cfg0["params"]
+    knots, y, coef = [t.cpu().numpy() for t in M.mbhl_sparse(ctx, dev(params))]
+    check_sparse_stage(table, params, knots, y, coef, cfg0["freqs"][0], cfg0["freqs"][-1], cfg0["S"], cfg0["t0"])
+    M.mbhl_free(ctx)
+
+
+@pytest.mark.parametrize("S", [512, 1024])
+def test_sparse_stage_parity_at_benchmark_knot_counts(table, S):
+    # The knot counts of BASELINE configs 1-4 (S a multiple of 32 up to 1024: the fast 32-row sweeps of k_sparse_spline), on
+    # config 3's own grid (T_obs = 1.33 yr, f up to 0.1 Hz) with 16 walkers from config 3's prior (M_T log-uniform 1e5-1e8 Msun,
+    # workloads.sparse_batch): bands that start at the grid's first bin, bands that end inside it, heavy binaries whose modes
+    # span barely a decade.  Same element-by-element bars as the S = 256 case above.
+    freqs = W.grid(1.33, int(0.1 * 1.33 * W.YEAR_JULIAN_S), 0.0)
+    n = freqs.size
+    ctx = M.mbhl_init(dev(freqs), torch.zeros((3, n, 2), dtype=torch.float64, device=DEV),
+                      torch.ones((3, n), dtype=torch.float64, device=DEV), sparse_points=S)
+    params = W.sparse_batch(16)
+    assert params[:, 0].min() < 1e6 < 1e7 < params[:, 0].max()              # light and heavy binaries both drawn
+    knots, y, coef = [t.cpu().numpy() for t in M.mbhl_sparse(ctx, dev(params))]
+    n_active = check_sparse_stage(table, params, knots, y, coef, freqs[0], freqs[-1], S, 0.0)
+    assert n_active >= 80                                                  # nearly all of the 96 (walker, mode) pairs are in band
+    f_hi = knots[:, :, -1]
+    assert np.any((f_hi > 0) & (f_hi < 0.99 * freqs[-1])) and np.any(f_hi > 0.99 * freqs[-1])   # bands ending inside / at the grid edge
     M.mbhl_free(ctx)
 
 
