@@ -203,7 +203,9 @@ void mbhl_pt_free(mbhl_pt* pt);
  * is taken piecewise parabolic on the coarse bins (values at a bin's first, centre and last frequency): exact for one
  * fine bin per coarse bin; otherwise the error of the sums falls at least with the cube of the coarse bin width (with its fourth power on bins that hold no band edge and no region boundary of the model: pinned on the oracle in tests/test_oracle_heterodyne.py); accurate for walkers whose phase stays within a fraction of a cycle of the reference's across a
  * coarse bin (the bulk of a posterior).  The band of a mode is taken to be the reference's; no spline is extrapolated.  d_h, h_h, logL [B]: device
- * pointers, any may be NULL; asynchronous on the context's stream.  The context must outlive the handle.            */
+ * pointers, any may be NULL.  Asynchronous on the context's stream EXCEPT when a batch is larger than any this handle has seen:
+ * its partial-sum buffer ([B][coarse-bin groups][2] doubles) then grows, which synchronises the stream and calls cudaFree /
+ * cudaMalloc; call once with the largest batch during set-up to keep later calls free of both.  The context must outlive the handle. */
 typedef struct mbhl_het mbhl_het;
 int  mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const int64_t* edges, int32_t n_coarse);
 int  mbhl_het_loglike(mbhl_het* het, const double* params, int64_t B, double* d_h, double* h_h, double* logL);

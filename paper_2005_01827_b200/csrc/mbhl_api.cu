@@ -683,7 +683,7 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
     const size_t o_cf = take((size_t)MBHL_NMODE * (S - 1) * kCoefStride * 8), o_ed = take((nb + 1) * 8), o_pt = take(nb * 6 * 8), o_rp = take((size_t)MBHL_NMODE * nb * 3 * 8), o_pr = take((size_t)MBHL_NMODE * nb * 4);
     const size_t o_a0 = take(kHetA * nb * 16), o_a1 = take(kHetA * nb * 16), o_a2 = take(kHetA * nb * 16);
     const size_t o_b0 = take(kHetB * nb * 16), o_b1 = take(kHetB * nb * 16), o_b2 = take(kHetB * nb * 16);
-    const size_t o_lf = take(MBHL_NMODE * 8), o_id = take(MBHL_NMODE * 8), o_ac = take(MBHL_NMODE * 4), o_lo = take(MBHL_NMODE * 8), o_hi = take(MBHL_NMODE * 8);
+    const size_t o_lf = take(MBHL_NMODE * 8), o_id = take(MBHL_NMODE * 8), o_lo = take(MBHL_NMODE * 8), o_hi = take(MBHL_NMODE * 8);
     if (cudaMalloc(&het->mem, off) != cudaSuccess) { cudaGetLastError(); het->mem = nullptr; return bail(fail(ctx, MBHL_ENOMEM, "mbhl_het_init: cudaMalloc")); }
     char* m = het->mem;
     if (cudaMemcpyAsync(m + o_wc, base + L.consts, sizeof(WalkerConst), cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
@@ -694,14 +694,12 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
         cudaStreamSynchronize(st) != cudaSuccess)
         return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: copies"));
     double lf[MBHL_NMODE], id[MBHL_NMODE], flo[MBHL_NMODE], fhi[MBHL_NMODE];
-    int ac[MBHL_NMODE];
     for (int i = 0; i < MBHL_NMODE; ++i) {
-        lf[i] = wc_host.mode[i].ln_flo; id[i] = wc_host.mode[i].inv_dlog; ac[i] = wc_host.mode[i].active;
+        lf[i] = wc_host.mode[i].ln_flo; id[i] = wc_host.mode[i].inv_dlog;
         flo[i] = wc_host.mode[i].f_lo; fhi[i] = wc_host.mode[i].f_hi;
     }
     if (cudaMemcpyAsync(m + o_lf, lf, sizeof(lf), cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(m + o_id, id, sizeof(id), cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(m + o_ac, ac, sizeof(ac), cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(m + o_lo, flo, sizeof(flo), cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(m + o_hi, fhi, sizeof(fhi), cudaMemcpyHostToDevice, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess)
         return bail(fail(ctx, MBHL_ECUDA, "mbhl_het_init: copies"));
@@ -711,7 +709,7 @@ int mbhl_het_init(mbhl_ctx* ctx, mbhl_het** out, const double* params_ref, const
     H.B0 = (double2*)(m + o_b0); H.B1 = (double2*)(m + o_b1); H.B2 = (double2*)(m + o_b2);
     H.S = S; H.n_b = n_coarse; H.mode_mask = ctx->mode_mask;
     het->E.pts = (const double*)(m + o_pt); het->E.ref_p4 = (const double*)(m + o_rp); het->E.present = (const int*)(m + o_pr);
-    het->E.ref_ln_flo = (const double*)(m + o_lf); het->E.ref_inv_dlog = (const double*)(m + o_id); het->E.ref_active = (const int*)(m + o_ac);
+    het->E.ref_ln_flo = (const double*)(m + o_lf); het->E.ref_inv_dlog = (const double*)(m + o_id);
     het->E.ref_f_lo = (const double*)(m + o_lo); het->E.ref_f_hi = (const double*)(m + o_hi);
     het->E.n_groups = (n_coarse + kHetEvalThreads - 1) / kHetEvalThreads;
     k_het_bin_points<<<(n_coarse + 127) / 128, 128, 0, st>>>(ctx->freqs, H.edges, n_coarse, H.ref_dw, H.ref_knots, H.ref_coef, S, ctx->mode_mask,

@@ -149,7 +149,7 @@ struct HetEvalArgs {
     const double* pts;          // [n_b][3][2] (f, ln f) at the first, centre and last frequency of every coarse bin
     const double* ref_p4;       // [6][n_b][3] the reference's phase there (quarter turns)
     const int* present;         // [6][n_b] mode in band throughout the coarse bin (else absent: contributes nothing)
-    const double* ref_ln_flo; const double* ref_inv_dlog; const int* ref_active;   // [6]
+    const double* ref_ln_flo; const double* ref_inv_dlog;   // [6]
     const double* ref_f_lo; const double* ref_f_hi;                               // [6] the reference's bands
     double* partials;           // [B][n_groups][2]
     int n_groups;               // ceil(n_b / kHetEvalThreads)

@@ -302,8 +302,8 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
                 double mm[8], bb[8];
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    const int r = min(r0 + k, S - 1);
-                    mm[k] = mls[pad_idx(r)];
+                    const int r = min(r0 + k, own1 - 1);     // stay inside this thread's own rows: the rows past own1 are a
+                    mm[k] = mls[pad_idx(r)];                 // neighbour's, who may be writing them (the values were never used)
                     bb[k] = aq[pad_idx(r)];
                 }
 #pragma unroll
@@ -337,7 +337,7 @@ k_sparse_spline(const WalkerConst* __restrict__ wc, int S, double* __restrict__ 
                 double cc[8], gg[8];
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    const int r = max(r0 - k, 0);
+                    const int r = max(r0 - k, own0);         // likewise: never read below this thread's first row
                     cc[k] = cps[pad_idx(r)];
                     gg[k] = aq[pad_idx(r)];
                 }
