@@ -18,7 +18,10 @@ moments A_n = sum_{k in b} w_c conj(d_c) E0_m x_k^n and B_n = sum_{k in b} w_c E
 (terms in x^3, x^4 dropped).  The summary data A, B are computed once per reference; a walker
 costs its sparse stage plus 3 n_b spline evaluations per mode.  The band of a mode is taken to be the reference's
 (the summary data hold it); where f_L or f_R lies outside the band common to walker and reference, r is taken at the
-nearest frequency inside it (no spline is ever extrapolated).  The coarse bins actually used are the caller's edges
+nearest frequency inside it (no spline is ever extrapolated) - but only on coarse bins that the walker's own band
+reaches: a coarse bin lying wholly outside the walker's band [f_lo, f_hi] of a mode gets r = 0 for that mode, as in the
+brute-force sums, where the mode contributes nothing there (reading H1, amended: moving all three points of such a bin to
+the band edge would give it a constant non-zero envelope, an error that does not shrink with the bin width).  The coarse bins actually used are the caller's edges
 REFINED by the reference's band edges (first in-band bin and one past the last of every mode), so that on every coarse
 bin a mode is either in band throughout or absent: without this the bins that hold a band edge dominate the error.
 With one fine bin per coarse bin the variant IS the
@@ -109,8 +112,10 @@ def _envelope(walker_modes, t_coal, summary, f):
         Phi0 = ospline.evaluate(ref["knots"], ref["coef"][:, 1, :], f)
         dth = TWO_PI * (_cycles(q[1], f, t_coal) - _cycles(Phi0, f, summary["ref_t_coal"]))
         e = q[0] * (np.cos(dth) + 1j * np.sin(dth))
+        # coarse bins (f has one entry per bin) that the walker's own band does not reach: the mode is absent there
+        reached = (summary["fR"] >= mo["knots"][0]) & (summary["fL"] <= mo["knots"][-1])
         for c in range(3):
-            r[c, m] = e * (q[2 + 2 * c] + 1j * q[3 + 2 * c])
+            r[c, m] = np.where(reached, e * (q[2 + 2 * c] + 1j * q[3 + 2 * c]), 0.0)
     return r
 
 

@@ -96,3 +96,25 @@ def test_order_of_convergence_on_a_window_without_band_edges_or_model_kinks(tabl
         assert e_dh[a] / e_dh[b] > 8.0, e_dh                   # at least third
     assert e_hh[0] / e_hh[3] > 512.0 and e_dh[0] / e_dh[3] > 512.0, (e_hh, e_dh)      # at least the cube over three halvings
     assert e_hh[0] < 1e-3 and e_hh[3] < 1e-6
+
+
+def test_coarse_bins_outside_the_walkers_own_band_contribute_nothing(table):
+    # Reading H1 (amended): a walker whose band starts LATER than the reference's (a smaller t_ref: every f_lo moves up) has no
+    # signal in the coarse bins between the two band edges; the brute-force sums skip those bins, so must the heterodyned ones.
+    # With one fine bin per coarse bin the parabola plays no role and the two must agree to rounding - before the amendment the
+    # bins in between carried the envelope of the band edge (a few bins per mode here, a relative error of ~1e-3).
+    wl = small_problem(table, n_bins=1500)
+    freqs = wl["freqs"]
+    inj = wl["injections"][0]
+    summ = H.setup(table, inj, freqs, wl["data"], wl["psd"], wl["S"], np.arange(freqs.size + 1))
+    walker = inj.copy()
+    walker[10] *= 0.97
+    ref_modes = L.sparse_stage(table, inj, freqs[0], freqs[-1], wl["S"])[0]
+    w_modes = L.sparse_stage(table, walker, freqs[0], freqs[-1], wl["S"])[0]
+    df = freqs[1] - freqs[0]
+    gaps = [(w["knots"][0] - r["knots"][0]) / df for w, r in zip(w_modes, ref_modes) if w is not None and r is not None]
+    assert min(gaps) > 1.5, gaps                       # every mode's band starts at least two fine bins later than the reference's
+    dh, hh, ll = H.loglike_parts(table, summ, walker)
+    rdh, rhh, rll = L.loglike_parts(table, walker, freqs, wl["data"], wl["psd"], wl["S"])
+    assert abs(hh - rhh) <= 1e-9 * rhh and abs(dh - rdh) <= 1e-9 * max(abs(rdh), rhh), (dh, rdh, hh, rhh)
+    assert abs(ll - rll) <= 1e-8 * (1.0 + abs(rll))
