@@ -202,7 +202,7 @@ void mbhl_pt_free(mbhl_pt* pt);
  * 3 n_coarse spline evaluations per mode, instead of one per fine bin.  The envelope A That exp(i (theta - theta_ref))
  * is taken piecewise parabolic on the coarse bins (values at a bin's first, centre and last frequency): exact for one
  * fine bin per coarse bin; otherwise the error of the sums falls at least with the cube of the coarse bin width (with its fourth power on bins that hold no band edge and no region boundary of the model: pinned on the oracle in tests/test_oracle_heterodyne.py); accurate for walkers whose phase stays within a fraction of a cycle of the reference's across a
- * coarse bin (the bulk of a posterior).  The band of a mode is taken to be the reference's; no spline is extrapolated.  d_h, h_h, logL [B]: device
+ * coarse bin (the bulk of a posterior).  The band of a mode is taken to be the reference's, and a coarse bin that the walker's own band of that mode does not reach contributes nothing, as in mbhl_loglike; no spline is extrapolated.  d_h, h_h, logL [B]: device
  * pointers, any may be NULL.  Asynchronous on the context's stream EXCEPT when a batch is larger than any this handle has seen:
  * its partial-sum buffer ([B][coarse-bin groups][2] doubles) then grows, which synchronises the stream and calls cudaFree /
  * cudaMalloc; call once with the largest batch during set-up to keep later calls free of both.  The context must outlive the handle. */

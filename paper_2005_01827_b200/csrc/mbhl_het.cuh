@@ -156,7 +156,7 @@ struct HetEvalArgs {
 };
 
 // grid (ceil(n_b / 128), B): thread = coarse bin, blockIdx.y = walker.  Per mode and evaluation point (first, centre, last
-// frequency of the bin, each moved into the band common to walker and reference) the channel-independent part
+// frequency of the bin, each moved into the band common to walker and reference; a bin the walker's band does not reach is skipped) the channel-independent part
 // A exp(i [theta - theta0]) is formed once; the three channels then differ by their transfer cubics only.
 __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
     __shared__ double s_red[2][kHetEvalThreads / 32];
@@ -178,6 +178,7 @@ __global__ void __launch_bounds__(kHetEvalThreads) k_het_eval(HetEvalArgs E) {
             if (!E.present[mi * n_b + b] || !E.wc[wkr].mode[mi].active) continue;
             const ModeConst& mc = E.wc[wkr].mode[mi];
             if (!(fmax(mc.f_lo, E.ref_f_lo[mi]) <= fmin(mc.f_hi, E.ref_f_hi[mi]))) continue;
+            if (f3[2] < mc.f_lo || f3[0] > mc.f_hi) continue;     // the walker's own band does not reach this coarse bin: no signal here (H1, amended)
             const double* x = E.knots + (wkr * MBHL_NMODE + mi) * S;
             const double* cbase = E.coef + (wkr * MBHL_NMODE + mi) * (int64_t)(S - 1) * kCoefStride;
 #pragma unroll

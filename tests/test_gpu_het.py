@@ -57,6 +57,36 @@ def test_het_parity_small(table):
     M.mbhl_free(ctx)
 
 
+def test_het_walker_with_a_band_that_starts_later_than_the_references(table):
+    # Reading H1 as amended in round 3: coarse bins that the walker's own band does not reach contribute nothing.  A walker with
+    # a smaller t_ref has every f_lo above the reference's.  GPU against the oracle on ragged coarse bins, and - with one fine
+    # bin per coarse bin, where the parabola plays no role - GPU heterodyne against the GPU brute-force path.
+    wl = W.build(0, lambda p, f, Sp: L.template(table, p, f, Sp), n_bins=1500, batch=4)
+    S = 64
+    freqs = wl["freqs"]
+    ctx = M.mbhl_init(dev(freqs), dev(wl["data"]), dev(wl["psd"]), sparse_points=S, t0=wl["t0"])
+    inj = wl["injections"][0]
+    shifted = inj.copy()
+    shifted[10] *= 0.97                                  # bands start a few fine bins later in every mode
+    later = inj.copy()
+    later[10] *= 0.999
+    walkers = np.stack([shifted, later, inj])
+    brute = [t.cpu().numpy() for t in M.mbhl_loglike_parts(ctx, dev(walkers))]
+    for nb in (64, freqs.size):
+        edges = W.het_edges(freqs, nb) if nb < freqs.size else np.arange(freqs.size + 1)
+        summ = H.setup(table, inj, freqs, wl["data"], wl["psd"], S, edges, wl["t0"])
+        het = M.mbhl_het_init(ctx, dev(inj), edges)
+        dh, hh, ll = [t.cpu().numpy() for t in M.mbhl_het_loglike(het, dev(walkers))]
+        for b in range(3):
+            rdh, rhh, rll = H.loglike_parts(table, summ, walkers[b])
+            assert abs(hh[b] - rhh) <= 1e-8 * rhh and abs(dh[b] - rdh) <= 1e-8 * max(abs(rdh), rhh), (nb, b, dh[b], rdh, hh[b], rhh)
+            assert abs(ll[b] - rll) <= 1e-6 * (1.0 + abs(rll)), (nb, b, ll[b], rll)
+            if nb == freqs.size:
+                assert abs(hh[b] - brute[1][b]) <= 1e-9 * brute[1][b] and abs(dh[b] - brute[0][b]) <= 1e-9 * max(abs(brute[0][b]), brute[1][b]), b
+        M.mbhl_het_free(het)
+    M.mbhl_free(ctx)
+
+
 def test_het_config2_scale_parity_and_accuracy(table):
     # config-2 grid (N = 4 197 160, S = 1024), reference = the 1e6 Msun injection, walkers at posterior-like distances
     wl = W.build(2, lambda p, f, S: L.template(table, p, f, S) if p[0] == 1e6 else np.zeros((3, f.size), dtype=np.complex128))
