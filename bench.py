@@ -41,6 +41,12 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 lanes 
 DENSE_TRAFFIC = {2: (2.0385e9, "profiles/r02_dense_c2_ncu.txt (dram__bytes_read.sum 2.0289 GB + dram__bytes_write.sum 9.6 MB)")}
 
 
+def _stage_dict(stage):
+    """Per-stage milliseconds by name.  Slot 2 of mbhl_stage_times (the former stand-alone spline kernel) is a zero-length
+    interval between two back-to-back event records since the spline solve was fused into the sparse kernel: not reported."""
+    return {k: float(stage[i]) for i, k in ((0, "consts"), (1, "sparse_spline_fused"), (3, "dense"), (4, "reduce"))}
+
+
 def executed_flops(counts):
     """FP64 FLOPs k_dense executed, from its own tallies (uniform, gated, per-bin-record calls; lane evaluations; epilogues)."""
     n_uni, n_gat, n_rec, n_lane, n_epi = counts
@@ -163,15 +169,15 @@ def run_reference(args):
     wl = pool.wl
     B, N, S = wl["params"].shape[0], wl["freqs"].size, wl["S"]
     idx = pool.sample(min(16, max(3, pool.cores)))
-    for _ in range(min(args.warmup, 1)):
-        pool.time(idx[:pool.cores])
+    for _ in range(args.warmup):                # W untimed passes over the same sample, as the contract asks
+        pool.time(idx)
     t = sum(pool.time(idx)[0] for _ in range(args.steps))
     pool.close()
     value = len(idx) * args.steps / t
     sample = f"{len(idx)} walkers {idx} of the batch per step (spread over the injection groups), full grid, one walker per process on {pool.cores} cores"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "logL/s", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, B, N, S), "sample": sample},
         "cpu_baseline": {"value": value, "unit": "logL/s", "cores": pool.cores, "kind": "oracle", "sample": sample},
@@ -212,8 +218,9 @@ def _hbm_peak():
         return 6650.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
 
 
-def run_sparse_isolation(args):
-    """BASELINE.json configs[3]: B = 16384 parameter sets, steps a1-a5 only (mbhl_sparse), no dense stage."""
+def run_sparse_isolation(args, collect=None):
+    """BASELINE.json configs[3]: B = 16384 parameter sets, steps a1-a5 only (mbhl_sparse), no dense stage.
+    collect: a list that receives the result line instead of stdout (the default run's `also` entry)."""
     torch, M, dev, local = _device_setup()
     from paper_2005_01827_b200 import workloads as W
     S, B = 1024, args.batch or 16384
@@ -249,7 +256,7 @@ def run_sparse_isolation(args):
     fp64_peak = _fp64_probe(torch, M, dev)
     flops_set = 1730.0 * 6 * S                                       # ~1600 + 130 FLOPs per knot
     hbm_ms, fp64_ms = B * bytes_set / (hbm * 1e9) * 1e3, B * flops_set / (fp64_peak * 1e12) * 1e3
-    print(json.dumps({
+    line = ({
         "metric": "parameter sets/sec (sparse stage only)", "value": B / (ms * 1e-3), "unit": "sets/s", "n_gpus": 1,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -262,12 +269,17 @@ def run_sparse_isolation(args):
                      "frac": max(fp64_ms, hbm_ms) / stage[1], "frac_of_step": max(fp64_ms, hbm_ms) / ms,
                      "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac_hbm": achieved / hbm,
                      "traffic": None, "peak_source": hbm_src, "algorithmic_bytes_per_launch": k_bytes,
-                     "whole_stage": {"hbm_bound_ms": hbm_ms, "fp64_bound_ms": fp64_ms, "measured_ms": ms, "fp64_peak_tflops": fp64_peak}}}))
+                     "whole_stage": {"hbm_bound_ms": hbm_ms, "fp64_bound_ms": fp64_ms, "measured_ms": ms, "fp64_peak_tflops": fp64_peak}}})
     M.mbhl_free(ctx)
+    if collect is not None:
+        collect.append(line)
+    else:
+        print(json.dumps(line))
 
 
-def run_dense_sweep(args):
-    """BASELINE.json configs[4]: dense grid N x batch B sweep, random priors with M_T log-uniform [1e5, 1e8]; one line per point."""
+def run_dense_sweep(args, collect=None):
+    """BASELINE.json configs[4]: dense grid N x batch B sweep, random priors with M_T log-uniform [1e5, 1e8]; one line per point.
+    collect: a list that receives the result lines instead of stdout (the default run's `also` entry)."""
     torch, M, dev, local = _device_setup()
     from paper_2005_01827_b200 import workloads as W
     S = 1024
@@ -315,16 +327,20 @@ def run_dense_sweep(args):
             # HBM lower bound: every walker tile (<= 8 walkers) streams at least its largest walker's bins once (80 B per bin),
             # and every record of an in-band interval is read once
             hbm_ms = (80.0 * bins / min(B, 8) + B * 6 * (S - 1) * 256) / (hbm * 1e9) * 1e3
-            print(json.dumps({"metric": METRIC, "value": B / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1, "steps": steps, "ms_per_step": ms,
+            line = ({"metric": METRIC, "value": B / (ms * 1e-3), "unit": "logL/s", "n_gpus": 1, "steps": steps, "ms_per_step": ms,
                               "dtype": "f64", "data": "synthetic",
                               "config": {"workload": f"BASELINE.json configs[4] point: N=2^{logn} bins ending at 0.1 Hz, B={B}, S={S}",
                                          "active_pairs_per_step": pairs, "active_bins_per_step": bins,
-                                         "stage_ms": {k: float(v) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
+                                         "stage_ms": _stage_dict(stage)},
                               "roofline": {"bound": "alu" if fp64_ms >= hbm_ms else "hbm", "dense_fp64_bound_ms": fp64_ms, "dense_hbm_bound_ms": hbm_ms,
                                            "frac": max(fp64_ms, hbm_ms) / stage[3], "frac_of_step": max(fp64_ms, hbm_ms) / ms,
                                            "flops_table": flops_table, "flops_executed": flops_exec, "fp64_peak_tflops": fp64_peak,
                                            "dense_work_counts": dict(zip(("uniform_calls", "gated_calls", "perbin_record_calls", "lane_evals", "epilogues"), counts))},
-                              "finite": bool(torch.isfinite(logL).all().item())}), flush=True)
+                              "finite": bool(torch.isfinite(logL).all().item())})
+            if collect is not None:
+                collect.append(line)
+            else:
+                print(json.dumps(line), flush=True)
         M.mbhl_free(ctx)
 
 
@@ -462,6 +478,64 @@ def run_het(args):
             for h in hets:
                 M.mbhl_het_free(h)
     M.mbhl_free(ctx)
+
+
+def _also_points(args, torch, M, dev, local, fp64_peak):
+    """The short BASELINE configs, measured after the headline's timed region and outside it, so that the one JSON line of
+    the default run carries them: config 3 (sparse-stage isolation, 5 steps), config 0 (B = 4, N = 2^16, 200 steps) and one
+    config-4 point (N = 2^16, B = 1024).  Each entry: ms_per_step, the roofline fraction of its dominant kernel, the bound."""
+    from types import SimpleNamespace
+    from paper_2005_01827_b200 import workloads as W
+    out = {}
+    got = []
+    run_sparse_isolation(SimpleNamespace(steps=5, warmup=3, batch=0), collect=got)
+    r = got[-1]
+    out["config3_sparse_isolation"] = {"ms_per_step": r["ms_per_step"], "frac": r["roofline"]["frac"], "bound": r["roofline"]["bound"],
+                                       "kernel": "k_sparse_spline", "unit_per_step": "16384 parameter sets"}
+    got = []
+    run_dense_sweep(SimpleNamespace(steps=20, warmup=3, batch=1024, logn=16), collect=got)
+    r = got[-1]
+    out["config4_N2^16_B1024"] = {"ms_per_step": r["ms_per_step"], "frac": r["roofline"]["frac"], "bound": r["roofline"]["bound"],
+                                  "kernel": "k_dense", "dense_ms": r["config"]["stage_ms"]["dense"]}
+    # config 0: latency-bound (four kernels of a few microseconds each); frac is that of k_dense like the headline's
+    state = {}
+
+    def gpu_template(p, f, S):
+        if "ctx0" not in state:
+            n = f.size
+            state["ctx0"] = M.mbhl_init(torch.as_tensor(f, device=dev), torch.zeros((3, n, 2), dtype=torch.float64, device=dev),
+                                        torch.ones((3, n), dtype=torch.float64, device=dev), sparse_points=S, device=local)
+        h = M.mbhl_template(state["ctx0"], torch.as_tensor(p[None, :].copy(), device=dev))
+        torch.cuda.synchronize()
+        return h[0].cpu().numpy()
+
+    wl = W.build(0, gpu_template)
+    M.mbhl_free(state.pop("ctx0"))
+    t = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=dev)
+    B = wl["params"].shape[0]
+    ctx = M.mbhl_init(t(wl["freqs"]), t(wl["data"]), t(wl["psd"]), sparse_points=wl["S"], t0=wl["t0"], max_batch=B, device=local)
+    params, logL = t(wl["params"]), torch.empty(B, dtype=torch.float64, device=dev)
+    M.mbhl_enable_stage_timing(ctx, True)
+    for _ in range(10):
+        M.mbhl_loglike(ctx, params, logL)
+    torch.cuda.synchronize()
+    steps, ms, dense = 200, 0.0, 0.0
+    M.mbhl_stage_times(ctx)                          # forget the warm-up calls
+    for _ in range(steps // 50):                     # the stage-event ring holds 64 calls: read (and reset) it every 50
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(50):
+            M.mbhl_loglike(ctx, params, logL)
+        e1.record()
+        torch.cuda.synchronize()
+        ms += e0.elapsed_time(e1) / steps
+        dense += M.mbhl_stage_times(ctx)[3] * 50 / steps
+    pairs, bins = M.mbhl_last_work(ctx)
+    flops, _, _ = dense_numerator(pairs, bins, M.mbhl_last_dense_work(ctx))
+    out["config0"] = {"ms_per_step": ms, "frac": flops / (dense * 1e-3) / 1e12 / fp64_peak, "bound": "latency (alu roofline of k_dense shown)",
+                      "kernel": "k_dense", "dense_ms": dense, "walkers": B, "bins": int(wl["freqs"].size)}
+    M.mbhl_free(ctx)
+    return out
 
 
 def run_ours(args):
@@ -653,7 +727,7 @@ def run_ours(args):
                                 else "every rank its own batch, data replicated, no data-path collective"),
                    "l2": "inputs larger than L2 (0.34 GB weighted data + 1.6 GB spline coefficients per step vs 126 MB L2)",
                    "active_pairs_per_step": pairs, "active_bins_per_step": bins,
-                   "stage_ms": {k: float(v / args.steps) for k, v in zip(("consts", "sparse", "spline", "dense", "reduce"), stage)}},
+                   "stage_ms": _stage_dict(stage / args.steps)},
         "e2e": {"value": n_job * args.steps / e2e_s, "unit": "logL/s", "h2d_bytes_per_step": int(n_rank * 11 * 8),
                 "d2h_bytes_per_step": int(n_rank * 8)},
         "gpu_launches": int(launches),
@@ -671,8 +745,10 @@ def run_ours(args):
     }
     if cpu is not None:
         out["cpu_baseline"] = cpu
-    print(json.dumps(out))
     M.mbhl_free(ctx)
+    if world == 1 and args.config == 2 and args.also:
+        out["also"] = _also_points(args, torch, M, dev, local, fp64_peak)
+    print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 
@@ -684,7 +760,8 @@ def spawn_ranks(args):
         sk.bind(("127.0.0.1", 0))
         port = sk.getsockname()[1]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")            # the communicator lines (ranks, NVLS) are evidence the driver reads
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
            "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
     raise SystemExit(subprocess.call(cmd, env=env))
@@ -707,6 +784,8 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=("weak", "strong"),
                     help="N > 1: weak = every rank its own batch of B walkers; strong = ONE batch sharded across the ranks (shard.py)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--no-also", dest="also", action="store_false",
+                    help="default run only: skip the short extra configs (3, 0, one config-4 point) reported under the key `also`")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.config > 2:
