@@ -42,3 +42,10 @@ def test_host_core_count_and_workload_name():
     b = load_bench()
     assert 1 <= b.host_cores() <= (os.cpu_count() or 1)
     assert "configs[2]" in b.workload_name(2, 1024, 4197160, 1024)
+
+
+def test_stage_dict_names_the_fused_kernel_and_drops_the_retired_slot():
+    # mbhl_stage_times keeps five slots for layout; slot 2 (the former stand-alone spline kernel) is a zero-length interval
+    import bench
+    d = bench._stage_dict([0.06, 0.88, 0.007, 58.5, 0.008])
+    assert d == {"consts": 0.06, "sparse_spline_fused": 0.88, "dense": 58.5, "reduce": 0.008}
