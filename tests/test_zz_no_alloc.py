@@ -64,7 +64,7 @@ def test_static_scratch_entry_point_matches_the_allocating_path_on_two_calls_in_
         before = torch.cuda.mem_get_info()[0]
         got = M.mbhl_unpack_coords_static(ctx, rows, coords, out)       # fixed-array path
         torch.cuda.synchronize()
-        assert torch.cuda.mem_get_info()[0] == before                   # the call took no device memory
+        assert torch.cuda.mem_get_info()[0] >= before                   # the call took no device memory
         np.testing.assert_array_equal(got.cpu().numpy(), want.cpu().numpy())   # bit for bit; NaN == NaN here
         assert np.all(np.isnan(got[0].cpu().numpy())) and np.all(np.isfinite(got[1:].cpu().numpy()))
     # and once more with the first batch: a repeat after the short call still agrees
